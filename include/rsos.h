@@ -1,0 +1,177 @@
+/*
+ * rsos.h -- C ABI of librsos: the B200 (sm_100a) hot path of the restricted solid-on-solid (RSOS)
+ * deposition Monte Carlo of arXiv 1605.02620 (Kelling, Odor, Gemming).
+ *
+ * Citations:  P:n = /root/reference/PAPER.md line n;  D:x = DESIGN.md section x (the seeded
+ * schedule DT(S,K) / RS restated from SURVEY.md 8(c).1, and the readings Q1..Q15 of the paper).
+ *
+ * What the library computes (Eq. 6): on a periodic L x L integer height lattice a site x
+ * is picked at random and h(x) += 1 is accepted iff afterwards |h(x) - h(x')| <= N for the four
+ * nearest neighbours x'.  R independent realizations are advanced at once; one Monte-Carlo
+ * step (MCS) is L*L attempts per realization (reading Q4).  Large lattices are updated by
+ * double tiling with a randomly moved origin: tiles of side S in four colour sets, one
+ * seeded origin per sub-sweep, S*S/K sequential attempts per tile per sub-sweep (D:2).  All random
+ * numbers come from Philox4x32-10 keyed by the seed with counter (call, tile, sub-sweep,
+ * realization), so a realization is a pure function of (seed, r, L, N, S, K).  The squared
+ * interface width W^2(L,t) (Eq. 2) is returned from exact integer sums.
+ *
+ * Conventions for every entry point
+ *   - plain C, no exceptions; returns RSOS_OK (0) or a negative RSOS_E* code, and a failed call
+ *     has no partial effect on the context (except after RSOS_ECUDA, when the context is dead);
+ *   - rsos_last_error() returns a thread-local, NUL-terminated message for the last failure;
+ *   - "host" pointers are ordinary CPU memory owned by the caller (pinned or pageable), "device"
+ *     pointers are CUDA global memory of the context's device;
+ *   - all work is enqueued on the context's stream; calls that return host data synchronise
+ *     that stream before returning, rsos_advance does not;
+ *   - a context is not thread-safe; distinct contexts are independent.
+ * There is no CPU fallback: without a CUDA device every call fails with RSOS_ECUDA.
+ */
+#ifndef RSOS_H
+#define RSOS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rsos_ctx rsos_ctx;
+
+enum {
+    RSOS_OK       =  0,
+    RSOS_EINVAL   = -1,   /* bad argument (message says which)                                   */
+    RSOS_ERANGE   = -2,   /* a counter would overflow: (t + mcs) * K >= 2^32, or sum h^2 >= 2^64 */
+    RSOS_ENOMEM   = -3,   /* host or device allocation failed                                    */
+    RSOS_ECUDA    = -4,   /* CUDA runtime error (message carries cudaGetErrorString)             */
+    RSOS_EUNSUP   = -5    /* the requested engine cannot run this configuration                  */
+};
+
+/* Update engines.  All of them produce bit-identical heights (tests/test_gpu_parity.py).       */
+enum {
+    RSOS_ENGINE_AUTO   = 0,  /* ONCHIP when the mode is RS and the lattice fits in shared memory, */
+                             /* else WARP in DT mode, else SIMPLE                                 */
+    RSOS_ENGINE_SIMPLE = 1,  /* one thread per active tile, heights in global memory (slow;       */
+                             /* the literal loop nest of D:2, kept as an on-device cross-check)   */
+    RSOS_ENGINE_WARP   = 2,  /* DT mode: one warp per active tile, (S+2)^2 window staged in       */
+                             /* shared memory, 32 attempts in flight with exact conflict votes    */
+    RSOS_ENGINE_ONCHIP = 3   /* RS mode (2S > L): one warp per realization, the whole lattice     */
+                             /* stays in shared memory for all MCS of one rsos_advance call       */
+};
+
+/* Options; all fields optional, zero = default.  Passed by pointer, copied by rsos_init.       */
+typedef struct rsos_opts {
+    uint32_t tile;        /* S: tile side, power of two >= 8; default 64.  2*S > L selects the    */
+                          /* serial random-sequential mode RS (one tile = the lattice) (D:2)      */
+    uint32_t subsweeps;   /* K: sub-sweeps per MCS, power of two, K | S*S, S*S/K >= 32; default 1 */
+    uint32_t first_real;  /* global index of realization 0 (a run may be split over contexts)     */
+    uint32_t engine;      /* RSOS_ENGINE_*                                                        */
+    int32_t *d_heights;   /* DEVICE: borrowed buffer of R*L*L int32 (h[r][y][x], row-major, 16-   */
+                          /* byte aligned), e.g. a torch tensor; NULL = the library allocates.    */
+                          /* Its content on entry is ignored: rsos_init zeroes it (flat start).   */
+    void    *stream;      /* cudaStream_t to enqueue on; NULL = the legacy default stream         */
+    int32_t  device;      /* CUDA device ordinal + 1; 0 = the current device                      */
+    uint32_t reserved;    /* must be 0                                                            */
+} rsos_opts;
+
+/*
+ * rsos_init -- create a context: R flat surfaces h = 0 at t = 0, accepted = 0.
+ *   ctx   out, host: receives the context (NULL on failure)
+ *   L     lattice side, power of two, 4 <= L <= 65536 (periodic in both directions, reading Q2)
+ *   N     height-difference bound of Eq. (6), 1 <= N <= 127
+ *   R     number of independent realizations, >= 1, R*L*L*4 bytes must fit on the device
+ *   seed  Philox key (low word, high word)
+ *   opts  host, may be NULL
+ * Errors: RSOS_EINVAL (L, N, R, tile, subsweeps, engine, misaligned d_heights), RSOS_EUNSUP
+ * (engine cannot run the mode), RSOS_ENOMEM, RSOS_ECUDA.
+ */
+int rsos_init(rsos_ctx **ctx, uint32_t L, uint32_t N, uint32_t R, uint64_t seed, const rsos_opts *opts);
+
+/*
+ * rsos_advance -- advance every realization by `mcs` Monte-Carlo steps of the schedule D:2
+ * (P:61-63 rule, P:77 decomposition): t += mcs.  Asynchronous: kernels are enqueued on the
+ * context's stream and the call returns.  mcs = 0 is a no-op.
+ * Errors: RSOS_ERANGE if (t + mcs) * K >= 2^32 (nothing is enqueued), RSOS_ECUDA.
+ */
+int rsos_advance(rsos_ctx *ctx, uint64_t mcs);
+
+/*
+ * rsos_sums -- exact integer sums per realization (Eq. 2):
+ *   S1[r] = sum_x h(x)  (int64),  S2[r] = sum_x h(x)^2  (uint64),  accepted[r] = accepted deposits.
+ * Host buffers of R elements each; any of them may be NULL.  Synchronises the stream.
+ * Errors: RSOS_ERANGE if max(h)^2 * L^2 could reach 2^64 (checked on the device), RSOS_ECUDA.
+ */
+int rsos_sums(rsos_ctx *ctx, int64_t *S1, uint64_t *S2, int64_t *accepted);
+
+/*
+ * rsos_width -- W2[r] = (L^2 * S2 - S1^2) / L^4 and hmean[r] = S1 / L^2 as doubles (Eq. 2), the
+ * numerator formed exactly in 128-bit integers and converted once (L^4 is a power of two, so W2
+ * is the correctly rounded exact value).  Host buffers of R doubles; either may be NULL.
+ * Synchronises the stream.  Errors as rsos_sums.
+ */
+int rsos_width(rsos_ctx *ctx, double *W2, double *hmean);
+
+/*
+ * rsos_moments -- (Eq. 13-15) exact central power sums about the
+ * integer base b[r] = floor(S1[r] / L^2):  M[r][k-1] = sum_x (h(x) - b[r])^k for k = 1..4 as
+ * signed 128-bit integers stored little-endian in two uint64 words (lo, hi): out[r][k-1][2].
+ * Host buffers: base (R int64, may be NULL) and out (R*4*2 uint64).  Synchronises the stream.
+ */
+int rsos_moments(rsos_ctx *ctx, int64_t *base, uint64_t *out);
+
+/*
+ * rsos_get_heights -- copy realizations r0 .. r0+nr-1 (nr*L*L int32, h[r][y][x]) to host_out.
+ * Synchronises the stream.  Errors: RSOS_EINVAL if the range is outside [0, R), RSOS_ECUDA.
+ */
+int rsos_get_heights(rsos_ctx *ctx, uint32_t r0, uint32_t nr, int32_t *host_out);
+
+/*
+ * rsos_set_state -- overwrite realizations r0 .. r0+nr-1 from host_in (same layout), set the sweep
+ * counter t (applies to all realizations) and, if accepted != NULL, their accepted counters
+ * (host, nr int64).  For snapshot restarts: t enters the Philox counter, so (heights, t) is the
+ * whole state.  The caller guarantees Eq. (6) holds in host_in.  Synchronises the stream.
+ */
+int rsos_set_state(rsos_ctx *ctx, uint32_t r0, uint32_t nr, const int32_t *host_in,
+                   uint64_t t, const int64_t *accepted);
+
+/* rsos_time -- *t = number of MCS done since the flat start (host pointer). */
+int rsos_time(rsos_ctx *ctx, uint64_t *t);
+
+/*
+ * rsos_info -- describe the context: out[0] = mode (0 RS, 1 DT), out[1] = engine in use,
+ * out[2] = S (effective tile side), out[3] = K, out[4] = kernel launches enqueued so far,
+ * out[5] = device SM count, out[6] = shared-memory bytes per block of the update kernel,
+ * out[7] = update-kernel blocks per launch.  Host buffer of 8 uint64.
+ */
+int rsos_info(rsos_ctx *ctx, uint64_t *out);
+
+/*
+ * rsos_device_heights -- *d = the DEVICE pointer of the height buffer (borrowed or owned), valid
+ * until rsos_free; reads of it must be ordered after the context's stream.
+ */
+int rsos_device_heights(rsos_ctx *ctx, int32_t **d);
+
+/*
+ * rsos_kernel_time -- accumulated device time of the update kernels, measured with CUDA events on
+ * the context's stream when timing was enabled with enable != 0 (it then records two events
+ * around every rsos_advance).  Synchronises the stream.  *ms_total and *n_launches (host) receive
+ * the totals since timing was enabled; enable = 0 switches it off.  Either pointer may be NULL.
+ */
+int rsos_kernel_time(rsos_ctx *ctx, int enable, double *ms_total, uint64_t *n_launches);
+
+/* rsos_free -- release the context and everything the library allocated (not d_heights). */
+void rsos_free(rsos_ctx *ctx);
+
+/* rsos_last_error -- message of the last failed call on this thread ("" if none). */
+const char *rsos_last_error(void);
+
+/*
+ * rsos_philox -- test hook: Philox4x32-10 of n (counter, key) pairs evaluated ON THE DEVICE by the
+ * same device function the update kernels use.  Host buffers: ctr (n*4 uint32), key (n*2 uint32),
+ * out (n*4 uint32).  Used to cross-check the generator against the oracle's and cuRAND's.
+ */
+int rsos_philox(const uint32_t *ctr, const uint32_t *key, uint32_t *out, uint32_t n);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RSOS_H */

@@ -1,0 +1,407 @@
+// rsos_api.cu -- the C ABI of librsos (include/rsos.h): argument checking, context, launch loops.
+// Product code (CUDA path).  No CPU fallback: every compute step runs in the kernels of
+// rsos_update.cu / rsos_reduce.cu.  Shares nothing with oracle/.
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "../../include/rsos.h"
+#include "rsos_device.cuh"
+#include "rsos_internal.h"
+
+using namespace rsos;
+
+struct rsos_ctx {
+    Params p;
+    bool mode_dt;
+    uint32_t engine;
+    uint64_t seed;
+    uint64_t t;
+    uint64_t launches;
+    int device;
+    cudaStream_t stream;
+    bool own_heights;
+    unsigned long long *d_red;        // R * 8 uint64 scratch for reductions
+    unsigned long long *h_red;        // pinned mirror
+    long long *d_base;                // R int64 (moments)
+    int sm_count;
+    size_t smem_bytes;
+    // optional timing of rsos_advance
+    bool timing;
+    cudaEvent_t ev0, ev1;
+    double ms_total;
+    uint64_t timed_launches;
+    uint64_t launches_at_ev0;
+    bool ev_pending;
+};
+
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                                   \
+    do {                                                                                                 \
+        cudaError_t e_ = (expr);                                                                         \
+        if (e_ != cudaSuccess) return fail(RSOS_ECUDA, "%s: %s", #expr, cudaGetErrorString(e_));         \
+    } while (0)
+
+static bool is_pow2(uint64_t v) { return v && !(v & (v - 1)); }
+static uint32_t ilog2(uint64_t v) { uint32_t l = 0; while ((1ull << l) < v) ++l; return l; }
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+        if (dev != prev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+extern "C" const char *rsos_last_error(void) { return g_err; }
+
+static void destroy(rsos_ctx *c)
+{
+    if (!c) return;
+    if (c->own_heights && c->p.h) cudaFree(c->p.h);
+    if (c->p.accepted) cudaFree(c->p.accepted);
+    if (c->p.err) cudaFree(c->p.err);
+    if (c->d_red) cudaFree(c->d_red);
+    if (c->h_red) cudaFreeHost(c->h_red);
+    if (c->d_base) cudaFree(c->d_base);
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
+    delete c;
+}
+
+extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uint64_t seed, const rsos_opts *o)
+{
+    if (!out) return fail(RSOS_EINVAL, "ctx is NULL");
+    *out = nullptr;
+    rsos_opts opt;
+    memset(&opt, 0, sizeof opt);
+    if (o) opt = *o;
+    if (!is_pow2(L) || L < 4 || L > 65536) return fail(RSOS_EINVAL, "L = %u must be a power of two in [4, 65536]", L);
+    if (N < 1 || N > 127) return fail(RSOS_EINVAL, "N = %u must be in [1, 127]", N);
+    if (R < 1) return fail(RSOS_EINVAL, "R must be >= 1");
+    if (opt.reserved) return fail(RSOS_EINVAL, "opts.reserved must be 0");
+    if (opt.engine > RSOS_ENGINE_ONCHIP) return fail(RSOS_EINVAL, "unknown engine %u", opt.engine);
+    uint32_t S = opt.tile ? opt.tile : 64, K = opt.subsweeps ? opt.subsweeps : 1;
+    if (!is_pow2(S) || S < 8) return fail(RSOS_EINVAL, "tile = %u must be a power of two >= 8", S);
+    if (!is_pow2(K)) return fail(RSOS_EINVAL, "subsweeps = %u must be a power of two", K);
+    const bool mode_dt = 2ull * S <= L;
+    if (mode_dt) {
+        if (((uint64_t)S * S) % K || (uint64_t)S * S / K < 32)
+            return fail(RSOS_EINVAL, "subsweeps = %u must divide tile^2 with tile^2/subsweeps >= 32", K);
+    } else {
+        S = L; K = 1;
+    }
+    if ((uintptr_t)opt.d_heights & 15u) return fail(RSOS_EINVAL, "d_heights must be 16-byte aligned");
+    if ((uint64_t)opt.first_real + R > 0xFFFFFFFFull) return fail(RSOS_EINVAL, "first_real + R overflows 32 bits");
+
+    // engine selection (include/rsos.h)
+    uint32_t engine = opt.engine;
+    const bool warp_ok = mode_dt && S <= 128 && N <= 31;
+    const bool onchip_ok = !mode_dt && L <= 128 && N <= 31;
+    if (engine == RSOS_ENGINE_AUTO) engine = mode_dt ? (warp_ok ? RSOS_ENGINE_WARP : RSOS_ENGINE_SIMPLE)
+                                                     : (onchip_ok ? RSOS_ENGINE_ONCHIP : RSOS_ENGINE_SIMPLE);
+    if (engine == RSOS_ENGINE_WARP && !warp_ok)
+        return fail(RSOS_EUNSUP, "engine WARP needs DT mode (2*tile <= L), tile <= 128 and N <= 31");
+    if (engine == RSOS_ENGINE_ONCHIP && !onchip_ok)
+        return fail(RSOS_EUNSUP, "engine ONCHIP needs RS mode (2*tile > L), L <= 128 and N <= 31");
+
+    int dev = 0;
+    if (opt.device > 0) dev = opt.device - 1;
+    else CUDA_TRY(cudaGetDevice(&dev));
+    DeviceGuard guard(dev);
+    if (!guard.ok) return fail(RSOS_ECUDA, "cannot select CUDA device %d", dev);
+
+    rsos_ctx *c = new (std::nothrow) rsos_ctx();
+    if (!c) return fail(RSOS_ENOMEM, "out of host memory");
+    memset(static_cast<void *>(c), 0, sizeof *c);
+    c->device = dev;
+    c->stream = (cudaStream_t)opt.stream;
+    c->mode_dt = mode_dt;
+    c->engine = engine;
+    c->seed = seed;
+    Params &p = c->p;
+    p.L = L; p.lgL = ilog2(L); p.N = N; p.R = R; p.first_real = opt.first_real;
+    p.S = S; p.lgS = ilog2(S); p.K = K;
+    p.k0 = (uint32_t)(seed & 0xFFFFFFFFull); p.k1 = (uint32_t)(seed >> 32);
+
+#define INIT_TRY(expr, code)                                                                             \
+    do {                                                                                                 \
+        cudaError_t e_ = (expr);                                                                         \
+        if (e_ != cudaSuccess) {                                                                         \
+            const int rc_ = fail(e_ == cudaErrorMemoryAllocation ? RSOS_ENOMEM : (code), "%s: %s", #expr, \
+                                 cudaGetErrorString(e_));                                                \
+            if (e_ == cudaErrorMemoryAllocation) cudaGetLastError();                                     \
+            destroy(c);                                                                                  \
+            return rc_;                                                                                  \
+        }                                                                                                \
+    } while (0)
+
+    const size_t bytes = (size_t)R * L * L * sizeof(int32_t);
+    if (opt.d_heights) { p.h = opt.d_heights; c->own_heights = false; }
+    else { INIT_TRY(cudaMalloc(&p.h, bytes), RSOS_ECUDA); c->own_heights = true; }
+    INIT_TRY(cudaMalloc(&p.accepted, (size_t)R * sizeof(unsigned long long)), RSOS_ECUDA);
+    INIT_TRY(cudaMalloc(&p.err, sizeof(uint32_t)), RSOS_ECUDA);
+    INIT_TRY(cudaMalloc(&c->d_red, (size_t)R * 8 * sizeof(unsigned long long)), RSOS_ECUDA);
+    INIT_TRY(cudaMallocHost(&c->h_red, (size_t)R * 8 * sizeof(unsigned long long)), RSOS_ECUDA);
+    INIT_TRY(cudaMalloc(&c->d_base, (size_t)R * sizeof(long long)), RSOS_ECUDA);
+    INIT_TRY(cudaMemsetAsync(p.h, 0, bytes, c->stream), RSOS_ECUDA);                 // flat start
+    INIT_TRY(cudaMemsetAsync(p.accepted, 0, (size_t)R * sizeof(unsigned long long), c->stream), RSOS_ECUDA);
+    INIT_TRY(cudaMemsetAsync(p.err, 0, sizeof(uint32_t), c->stream), RSOS_ECUDA);
+    INIT_TRY(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev), RSOS_ECUDA);
+    INIT_TRY(configure_engine(p, engine, mode_dt), RSOS_ECUDA);
+    INIT_TRY(cudaEventCreate(&c->ev0), RSOS_ECUDA);
+    INIT_TRY(cudaEventCreate(&c->ev1), RSOS_ECUDA);
+    c->smem_bytes = engine == RSOS_ENGINE_WARP ? warp_dt_smem(p.lgS) : engine == RSOS_ENGINE_ONCHIP ? warp_rs_smem(p.lgL) : 0;
+#undef INIT_TRY
+    *out = c;
+    return RSOS_OK;
+}
+
+extern "C" void rsos_free(rsos_ctx *c)
+{
+    if (!c) return;
+    DeviceGuard guard(c->device);
+    cudaStreamSynchronize(c->stream);
+    destroy(c);
+}
+
+static int flush_timing(rsos_ctx *c)
+{
+    if (c->timing && c->ev_pending) {
+        CUDA_TRY(cudaEventSynchronize(c->ev1));
+        float ms = 0.f;
+        CUDA_TRY(cudaEventElapsedTime(&ms, c->ev0, c->ev1));
+        c->ms_total += ms;
+        c->timed_launches += c->launches - c->launches_at_ev0;
+        c->ev_pending = false;
+    }
+    return RSOS_OK;
+}
+
+extern "C" int rsos_advance(rsos_ctx *c, uint64_t mcs)
+{
+    if (!c) return fail(RSOS_EINVAL, "ctx is NULL");
+    if (mcs == 0) return RSOS_OK;
+    const Params &p = c->p;
+    if (mcs >= (1ull << 32) || (c->t + mcs) * p.K >= (1ull << 32))
+        return fail(RSOS_ERANGE, "(t + mcs) * K = (%llu + %llu) * %u reaches 2^32", (unsigned long long)c->t,
+                    (unsigned long long)mcs, p.K);
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return fail(RSOS_ECUDA, "cannot select CUDA device %d", c->device);
+    if (c->timing) {
+        const int rc = flush_timing(c);
+        if (rc) return rc;
+        CUDA_TRY(cudaEventRecord(c->ev0, c->stream));
+        c->launches_at_ev0 = c->launches;
+    }
+    if (c->mode_dt) {
+        for (uint64_t m = 0; m < mcs; ++m)
+            for (uint32_t k = 0; k < p.K; ++k) {
+                const uint32_t u = (uint32_t)((c->t + m) * p.K + k);
+                for (uint32_t colour = 0; colour < 4; ++colour) {
+                    CUDA_TRY(launch_dt_pass(p, c->engine, u, colour, c->stream));
+                    ++c->launches;
+                }
+            }
+    } else {
+        CUDA_TRY(launch_rs_sweeps(p, c->engine, (uint32_t)c->t, (uint32_t)mcs, c->stream));
+        ++c->launches;
+    }
+    if (c->timing) {
+        CUDA_TRY(cudaEventRecord(c->ev1, c->stream));
+        c->ev_pending = true;
+    }
+    c->t += mcs;
+    return RSOS_OK;
+}
+
+static int check_device_err(rsos_ctx *c)
+{
+    uint32_t e = 0;
+    CUDA_TRY(cudaMemcpyAsync(&e, c->p.err, sizeof e, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    if (e) return fail(RSOS_ECUDA, "device-side consistency check failed (flags 0x%x)", e);
+    return RSOS_OK;
+}
+
+static int reduce_sums(rsos_ctx *c)
+{
+    const Params &p = c->p;
+    CUDA_TRY(launch_sums(p.h, p.L, p.R, c->d_red, c->stream));
+    c->launches += (p.R + 65534) / 65535;
+    CUDA_TRY(cudaMemcpyAsync(c->h_red, c->d_red, (size_t)p.R * 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaMemcpyAsync(c->h_red + (size_t)p.R * 4, p.accepted, (size_t)p.R * sizeof(unsigned long long),
+                             cudaMemcpyDeviceToHost, c->stream));
+    int rc = check_device_err(c);
+    if (rc) return rc;
+    // sum h^2 must stay below 2^64: max|h|^2 * L^2 < 2^64
+    for (uint32_t r = 0; r < p.R; ++r) {
+        const unsigned __int128 mx = c->h_red[4 * (size_t)r + 2];
+        if (mx * mx * ((unsigned __int128)p.L * p.L) >> 64)
+            return fail(RSOS_ERANGE, "realization %u: max|h| = %llu makes sum h^2 overflow 64 bits", r,
+                        (unsigned long long)mx);
+    }
+    return RSOS_OK;
+}
+
+extern "C" int rsos_sums(rsos_ctx *c, int64_t *S1, uint64_t *S2, int64_t *accepted)
+{
+    if (!c) return fail(RSOS_EINVAL, "ctx is NULL");
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return fail(RSOS_ECUDA, "cannot select CUDA device %d", c->device);
+    const int rc = reduce_sums(c);
+    if (rc) return rc;
+    const uint32_t R = c->p.R;
+    for (uint32_t r = 0; r < R; ++r) {
+        if (S1) S1[r] = (int64_t)c->h_red[4 * (size_t)r];
+        if (S2) S2[r] = c->h_red[4 * (size_t)r + 1];
+        if (accepted) accepted[r] = (int64_t)c->h_red[4 * (size_t)R + r];
+    }
+    return RSOS_OK;
+}
+
+extern "C" int rsos_width(rsos_ctx *c, double *W2, double *hmean)
+{
+    if (!c) return fail(RSOS_EINVAL, "ctx is NULL");
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return fail(RSOS_ECUDA, "cannot select CUDA device %d", c->device);
+    const int rc = reduce_sums(c);
+    if (rc) return rc;
+    const uint32_t R = c->p.R;
+    const unsigned __int128 n = (unsigned __int128)c->p.L * c->p.L;
+    const double nd = (double)c->p.L * (double)c->p.L;
+    for (uint32_t r = 0; r < R; ++r) {
+        const int64_t s1 = (int64_t)c->h_red[4 * (size_t)r];
+        const uint64_t s2 = c->h_red[4 * (size_t)r + 1];
+        const unsigned __int128 a1 = (unsigned __int128)(s1 < 0 ? -(__int128)s1 : (__int128)s1);
+        const unsigned __int128 num = n * s2 - a1 * a1;              // >= 0 (Cauchy-Schwarz)
+        if (W2) W2[r] = (double)num / (nd * nd);
+        if (hmean) hmean[r] = (double)s1 / nd;
+    }
+    return RSOS_OK;
+}
+
+extern "C" int rsos_moments(rsos_ctx *c, int64_t *base, uint64_t *out)
+{
+    if (!c) return fail(RSOS_EINVAL, "ctx is NULL");
+    if (!out) return fail(RSOS_EINVAL, "out is NULL");
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return fail(RSOS_ECUDA, "cannot select CUDA device %d", c->device);
+    int rc = reduce_sums(c);
+    if (rc) return rc;
+    const Params &p = c->p;
+    long long *hb = reinterpret_cast<long long *>(c->h_red + (size_t)p.R * 5);
+    for (uint32_t r = 0; r < p.R; ++r) {
+        const int64_t s1 = (int64_t)c->h_red[4 * (size_t)r];
+        hb[r] = s1 >> (2 * p.lgL);                                  // floor(S1 / L^2)
+        if (base) base[r] = hb[r];
+    }
+    CUDA_TRY(cudaMemcpyAsync(c->d_base, hb, (size_t)p.R * sizeof(long long), cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(launch_moments(p.h, p.L, p.R, c->d_base, c->d_red, c->stream));
+    c->launches += (p.R + 65534) / 65535;
+    CUDA_TRY(cudaMemcpyAsync(out, c->d_red, (size_t)p.R * 8 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    return RSOS_OK;
+}
+
+extern "C" int rsos_get_heights(rsos_ctx *c, uint32_t r0, uint32_t nr, int32_t *host_out)
+{
+    if (!c) return fail(RSOS_EINVAL, "ctx is NULL");
+    if ((uint64_t)r0 + nr > c->p.R) return fail(RSOS_EINVAL, "realizations [%u, %u) outside [0, %u)", r0, r0 + nr, c->p.R);
+    if (nr && !host_out) return fail(RSOS_EINVAL, "host_out is NULL");
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return fail(RSOS_ECUDA, "cannot select CUDA device %d", c->device);
+    const size_t per = (size_t)c->p.L * c->p.L;
+    if (nr) CUDA_TRY(cudaMemcpyAsync(host_out, c->p.h + r0 * per, nr * per * sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));
+    return check_device_err(c);
+}
+
+extern "C" int rsos_set_state(rsos_ctx *c, uint32_t r0, uint32_t nr, const int32_t *host_in, uint64_t t,
+                              const int64_t *accepted)
+{
+    if (!c) return fail(RSOS_EINVAL, "ctx is NULL");
+    if ((uint64_t)r0 + nr > c->p.R) return fail(RSOS_EINVAL, "realizations [%u, %u) outside [0, %u)", r0, r0 + nr, c->p.R);
+    if (nr && !host_in) return fail(RSOS_EINVAL, "host_in is NULL");
+    if (t * c->p.K >= (1ull << 32)) return fail(RSOS_ERANGE, "t * K reaches 2^32");
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return fail(RSOS_ECUDA, "cannot select CUDA device %d", c->device);
+    const size_t per = (size_t)c->p.L * c->p.L;
+    if (nr) CUDA_TRY(cudaMemcpyAsync(c->p.h + r0 * per, host_in, nr * per * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
+    if (nr && accepted)
+        CUDA_TRY(cudaMemcpyAsync(c->p.accepted + r0, accepted, nr * sizeof(int64_t), cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    c->t = t;
+    return RSOS_OK;
+}
+
+extern "C" int rsos_time(rsos_ctx *c, uint64_t *t)
+{
+    if (!c || !t) return fail(RSOS_EINVAL, "NULL argument");
+    *t = c->t;
+    return RSOS_OK;
+}
+
+extern "C" int rsos_info(rsos_ctx *c, uint64_t *out)
+{
+    if (!c || !out) return fail(RSOS_EINVAL, "NULL argument");
+    out[0] = c->mode_dt ? 1 : 0;
+    out[1] = c->engine;
+    out[2] = c->p.S;
+    out[3] = c->p.K;
+    out[4] = c->launches;
+    out[5] = (uint64_t)c->sm_count;
+    out[6] = c->smem_bytes;
+    out[7] = engine_blocks(c->p, c->engine, c->mode_dt);
+    return RSOS_OK;
+}
+
+extern "C" int rsos_device_heights(rsos_ctx *c, int32_t **d)
+{
+    if (!c || !d) return fail(RSOS_EINVAL, "NULL argument");
+    *d = c->p.h;
+    return RSOS_OK;
+}
+
+extern "C" int rsos_kernel_time(rsos_ctx *c, int enable, double *ms_total, uint64_t *n_launches)
+{
+    if (!c) return fail(RSOS_EINVAL, "ctx is NULL");
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return fail(RSOS_ECUDA, "cannot select CUDA device %d", c->device);
+    const int rc = flush_timing(c);
+    if (rc) return rc;
+    if (ms_total) *ms_total = c->ms_total;
+    if (n_launches) *n_launches = c->timed_launches;
+    if (enable && !c->timing) { c->timing = true; c->ms_total = 0; c->timed_launches = 0; c->ev_pending = false; }
+    if (!enable) c->timing = false;
+    return RSOS_OK;
+}
+
+extern "C" int rsos_philox(const uint32_t *ctr, const uint32_t *key, uint32_t *out, uint32_t n)
+{
+    if (n == 0) return RSOS_OK;
+    if (!ctr || !key || !out) return fail(RSOS_EINVAL, "NULL argument");
+    uint32_t *d = nullptr;
+    CUDA_TRY(cudaMalloc(&d, (size_t)n * 10 * sizeof(uint32_t)));
+    cudaError_t e = cudaMemcpy(d, ctr, (size_t)n * 4 * sizeof(uint32_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(d + (size_t)n * 4, key, (size_t)n * 2 * sizeof(uint32_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = launch_philox(d, d + (size_t)n * 4, d + (size_t)n * 6, n, nullptr);
+    if (e == cudaSuccess) e = cudaMemcpy(out, d + (size_t)n * 6, (size_t)n * 4 * sizeof(uint32_t), cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    if (e != cudaSuccess) return fail(RSOS_ECUDA, "rsos_philox: %s", cudaGetErrorString(e));
+    return RSOS_OK;
+}

@@ -1,0 +1,61 @@
+// rsos_device.cuh -- device-side building blocks shared by the update kernels of librsos.
+// Product code (CUDA path).  Shares nothing with oracle/.
+//
+// Citations: P:n = PAPER.md line n; D:x = DESIGN.md section x.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace rsos {
+
+// ---------------------------------------------------------------------------------------------
+// Philox4x32-10 (Salmon et al., SC'11), counter (c0..c3), key (k0,k1).  D:2 step 2.
+// Written for the GPU: the two 32x32->64 products are IMAD.WIDE, the key schedule is folded into
+// compile-time multiples of the Weyl constants so each round is 2 wide multiplies + 2 LOP3.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                                uint32_t k0, uint32_t k1)
+{
+    constexpr uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+    constexpr uint32_t W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+#pragma unroll
+    for (int i = 0; i < 10; ++i) {
+        const uint64_t p0 = (uint64_t)M0 * c0;
+        const uint64_t p1 = (uint64_t)M1 * c2;
+        const uint32_t ka = k0 + (uint32_t)i * W0;          // constant-folded offsets
+        const uint32_t kb = k1 + (uint32_t)i * W1;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ ka;
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ kb;
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
+// Everything a kernel needs to know about the run (passed by value).
+struct Params {
+    int32_t *h;                     // R * L * L heights, h[r][y][x]
+    unsigned long long *accepted;   // R accepted-deposit counters
+    uint32_t L, lgL;                // lattice side (power of two)
+    uint32_t N;                     // Eq. (6) bound
+    uint32_t R, first_real;
+    uint32_t S, lgS, K;             // tile side, sub-sweeps per MCS (DT); S = L, K = 1 in RS mode
+    uint32_t k0, k1;                // Philox key = (seed lo, seed hi)
+    uint32_t *err;                  // device error word (bit flags), see ERR_*
+};
+
+enum : uint32_t {
+    ERR_RECONSTRUCT = 1u,           // on-chip engine: height reconstruction did not divide exactly
+};
+
+// D:2 step 4: origin of sub-sweep u for realization rg: Philox counter (0, 0xFFFFFFFF, u, rg).
+__device__ __forceinline__ void draw_origin(const Params &p, uint32_t u, uint32_t rg, uint32_t &ox, uint32_t &oy)
+{
+    const uint4 o = philox4x32_10(0u, 0xFFFFFFFFu, u, rg, p.k0, p.k1);
+    ox = o.x & (p.L - 1);
+    oy = o.y & (p.L - 1);
+}
+
+}  // namespace rsos

@@ -1,0 +1,33 @@
+// rsos_internal.h -- host-side declarations shared by the translation units of librsos.
+// Product code (CUDA path).  Not part of the public ABI (that is include/rsos.h).
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace rsos {
+
+struct Params;
+
+constexpr int WARP_DT_WARPS = 8;     // warps (= tiles) per block of the DT warp engine
+constexpr int WARP_RS_WARPS = 4;     // warps (= realizations) per block of the on-chip RS engine
+
+enum : uint32_t { ENGINE_AUTO = 0, ENGINE_SIMPLE = 1, ENGINE_WARP = 2, ENGINE_ONCHIP = 3 };
+
+// rsos_update.cu
+size_t warp_dt_smem(uint32_t lgS);
+size_t warp_rs_smem(uint32_t lgL);
+cudaError_t configure_engine(const Params &p, uint32_t engine, bool mode_dt);
+uint32_t engine_blocks(const Params &p, uint32_t engine, bool mode_dt);
+cudaError_t launch_dt_pass(const Params &p, uint32_t engine, uint32_t u, uint32_t colour, cudaStream_t st);
+cudaError_t launch_rs_sweeps(const Params &p, uint32_t engine, uint32_t t0, uint32_t mcs, cudaStream_t st);
+cudaError_t launch_philox(const uint32_t *d_ctr, const uint32_t *d_key, uint32_t *d_out, uint32_t n, cudaStream_t st);
+
+// rsos_reduce.cu
+// out: per realization 4 x uint64: S1 (as int64 bits), S2, max |h| (max over threads), unused
+cudaError_t launch_sums(const int32_t *h, uint32_t L, uint32_t R, unsigned long long *d_out, cudaStream_t st);
+// out: per realization 8 x uint64: M1..M4 as (lo, hi) two's-complement 128-bit
+cudaError_t launch_moments(const int32_t *h, uint32_t L, uint32_t R, const long long *d_base,
+                           unsigned long long *d_out, cudaStream_t st);
+
+}  // namespace rsos

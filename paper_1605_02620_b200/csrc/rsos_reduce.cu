@@ -1,0 +1,140 @@
+// rsos_reduce.cu -- width reductions (sm_100a).  Product code; shares nothing with oracle/.
+//
+// Eq. (2): W^2 = (1/L^2) sum h^2 - ((1/L^2) sum h)^2 per realization.  The kernels return
+// exact integers S1 = sum h (int64) and S2 = sum h^2 (uint64); the division happens once on the
+// host from a 128-bit numerator (rsos_api.cu).  Integer adds commute, so the block order and the
+// atomics do not affect the result.  HBM-bound: 4 B per site, int4 loads, grid = multiple of SMs.
+#include "rsos_internal.h"
+
+namespace rsos {
+
+constexpr int RED_THREADS = 256;
+
+__global__ void __launch_bounds__(RED_THREADS) sums_kernel(const int32_t *__restrict__ h, uint32_t n4 /* L*L/4 */,
+                                                           unsigned long long *out)
+{
+    const uint32_t r = blockIdx.y;
+    const int4 *src = reinterpret_cast<const int4 *>(h) + (size_t)r * n4;
+    long long s1 = 0;
+    unsigned long long s2 = 0;
+    unsigned int mx = 0;
+    for (uint32_t i = blockIdx.x * RED_THREADS + threadIdx.x; i < n4; i += gridDim.x * RED_THREADS) {
+        const int4 q = __ldg(src + i);
+        s1 += (long long)q.x + (long long)q.y + (long long)q.z + (long long)q.w;
+        s2 += (unsigned long long)((long long)q.x * q.x) + (unsigned long long)((long long)q.y * q.y) +
+              (unsigned long long)((long long)q.z * q.z) + (unsigned long long)((long long)q.w * q.w);
+        mx = max(max(mx, (unsigned int)abs(q.x)), max((unsigned int)abs(q.y), max((unsigned int)abs(q.z), (unsigned int)abs(q.w))));
+    }
+    for (int o = 16; o; o >>= 1) {
+        s1 += __shfl_xor_sync(0xFFFFFFFFu, s1, o);
+        s2 += __shfl_xor_sync(0xFFFFFFFFu, s2, o);
+        mx = max(mx, __shfl_xor_sync(0xFFFFFFFFu, mx, o));
+    }
+    __shared__ long long w1[RED_THREADS / 32];
+    __shared__ unsigned long long w2[RED_THREADS / 32];
+    __shared__ unsigned int wm[RED_THREADS / 32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (lane == 0) { w1[warp] = s1; w2[warp] = s2; wm[warp] = mx; }
+    __syncthreads();
+    if (warp == 0) {
+        s1 = lane < RED_THREADS / 32 ? w1[lane] : 0;
+        s2 = lane < RED_THREADS / 32 ? w2[lane] : 0;
+        mx = lane < RED_THREADS / 32 ? wm[lane] : 0;
+        for (int o = 4; o; o >>= 1) {
+            s1 += __shfl_xor_sync(0xFFFFFFFFu, s1, o);
+            s2 += __shfl_xor_sync(0xFFFFFFFFu, s2, o);
+            mx = max(mx, __shfl_xor_sync(0xFFFFFFFFu, mx, o));
+        }
+        if (lane == 0) {
+            atomicAdd(out + 4 * r + 0, (unsigned long long)s1);      // two's complement: exact mod 2^64
+            atomicAdd(out + 4 * r + 1, s2);
+            atomicMax(out + 4 * r + 2, (unsigned long long)mx);
+        }
+    }
+}
+
+cudaError_t launch_sums(const int32_t *h, uint32_t L, uint32_t R, unsigned long long *d_out, cudaStream_t st)
+{
+    cudaError_t e = cudaMemsetAsync(d_out, 0, (size_t)R * 4 * sizeof(unsigned long long), st);
+    if (e != cudaSuccess) return e;
+    const uint64_t n4 = (uint64_t)L * L / 4;
+    // enough blocks per realization to cover 148 SMs x 8 blocks, at most one block per 256*4 int4
+    uint64_t bx = (n4 + RED_THREADS * 4 - 1) / (RED_THREADS * 4);
+    const uint64_t want = (148 * 8 + R - 1) / R;
+    if (bx > want) bx = want;
+    if (bx < 1) bx = 1;
+    for (uint32_t r0 = 0; r0 < R; r0 += 65535) {
+        const uint32_t nr = R - r0 < 65535 ? R - r0 : 65535;
+        sums_kernel<<<dim3((unsigned)bx, nr), RED_THREADS, 0, st>>>(h + (size_t)r0 * L * L, (uint32_t)n4, d_out + 4 * (size_t)r0);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Central power sums about an integer base b[r] (Eq. 13-15): M_k = sum (h - b)^k,
+// k = 1..4, exact in 128-bit two's complement.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void add128(unsigned long long *dst, __int128 v)
+{
+    const unsigned long long lo = (unsigned long long)v, hi = (unsigned long long)(v >> 64);
+    const unsigned long long old = atomicAdd(dst, lo);
+    const unsigned long long carry = (old + lo < old) ? 1ull : 0ull;
+    if (hi + carry) atomicAdd(dst + 1, hi + carry);
+}
+
+__device__ __forceinline__ __int128 shfl_xor128(__int128 v, int o)
+{
+    unsigned long long lo = (unsigned long long)v, hi = (unsigned long long)(v >> 64);
+    lo = __shfl_xor_sync(0xFFFFFFFFu, lo, o);
+    hi = __shfl_xor_sync(0xFFFFFFFFu, hi, o);
+    return (__int128)(((unsigned __int128)hi << 64) | lo);
+}
+
+__global__ void __launch_bounds__(RED_THREADS) moments_kernel(const int32_t *__restrict__ h, uint32_t n4,
+                                                              const long long *__restrict__ base, unsigned long long *out)
+{
+    const uint32_t r = blockIdx.y;
+    const int4 *src = reinterpret_cast<const int4 *>(h) + (size_t)r * n4;
+    const long long b = base[r];
+    __int128 m[4] = {0, 0, 0, 0};
+    for (uint32_t i = blockIdx.x * RED_THREADS + threadIdx.x; i < n4; i += gridDim.x * RED_THREADS) {
+        const int4 q = __ldg(src + i);
+        const int v[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const __int128 d = (long long)v[k] - b;
+            const __int128 d2 = d * d;
+            m[0] += d; m[1] += d2; m[2] += d2 * d; m[3] += d2 * d2;
+        }
+    }
+    for (int o = 16; o; o >>= 1)
+#pragma unroll
+        for (int k = 0; k < 4; ++k) m[k] += shfl_xor128(m[k], o);
+    if ((threadIdx.x & 31) == 0)
+#pragma unroll
+        for (int k = 0; k < 4; ++k) add128(out + 8 * r + 2 * k, m[k]);
+}
+
+cudaError_t launch_moments(const int32_t *h, uint32_t L, uint32_t R, const long long *d_base,
+                           unsigned long long *d_out, cudaStream_t st)
+{
+    cudaError_t e = cudaMemsetAsync(d_out, 0, (size_t)R * 8 * sizeof(unsigned long long), st);
+    if (e != cudaSuccess) return e;
+    const uint64_t n4 = (uint64_t)L * L / 4;
+    uint64_t bx = (n4 + RED_THREADS * 4 - 1) / (RED_THREADS * 4);
+    const uint64_t want = (148 * 8 + R - 1) / R;
+    if (bx > want) bx = want;
+    if (bx < 1) bx = 1;
+    for (uint32_t r0 = 0; r0 < R; r0 += 65535) {
+        const uint32_t nr = R - r0 < 65535 ? R - r0 : 65535;
+        moments_kernel<<<dim3((unsigned)bx, nr), RED_THREADS, 0, st>>>(h + (size_t)r0 * L * L, (uint32_t)n4, d_base + r0,
+                                                                       d_out + 8 * (size_t)r0);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
+}  // namespace rsos

@@ -1,0 +1,521 @@
+// rsos_update.cu -- the RSOS update kernels (sm_100a).  Product code; shares nothing with oracle/.
+//
+// Citations: P:n = PAPER.md line n; D:x = DESIGN.md section x.
+//
+// Three engines, all executing the seeded schedule of D:2 (RSOS rule P:61-63 Eq. 6, double tiling
+// with a moving origin P:77, independent realizations P:75) and producing identical heights:
+//
+//   simple_*   one THREAD per active tile, heights in global memory, the literal loop nest.
+//   warp_dt    one WARP per active tile.  The (S+2)^2 window is staged into shared memory as
+//              6-bit heights (mod 64) in 2x2-site blocks per 32-bit word, 32 consecutive attempts
+//              are evaluated at once and committed as the longest conflict-free prefix, so the
+//              result equals the sequential one exactly (D:4).
+//   warp_rs    RS mode: one warp per realization, the whole periodic lattice stays in shared
+//              memory for all MCS of the call (D:4, "on-chip").
+#include "rsos_device.cuh"
+#include "rsos_internal.h"
+
+namespace rsos {
+
+// =============================================================================================
+// SIMPLE engine: the literal loop nest of D:2 step 6, one thread per tile.
+// =============================================================================================
+__device__ __forceinline__ uint32_t simple_run_tile(const Params &p, int32_t *h, uint32_t rg, uint32_t u,
+                                                    uint32_t tile_id, uint32_t x0, uint32_t y0,
+                                                    uint32_t Se, uint32_t lgSe, uint64_t A)
+{
+    const uint32_t L = p.L, Lm = L - 1;
+    const uint32_t w16 = (2 * lgSe <= 16);
+    const uint32_t lg_ns = w16 ? 3 : 2;
+    const int32_t N = (int32_t)p.N;
+    uint32_t nacc = 0;
+    uint4 o = make_uint4(0, 0, 0, 0);
+    uint32_t have_q = 0xFFFFFFFFu;
+    for (uint64_t a = 0; a < A; ++a) {
+        const uint32_t lane = (uint32_t)a & 31u;
+        const uint32_t batch = (uint32_t)(a >> 5);
+        const uint32_t q = 32u * (batch >> lg_ns) + lane;
+        const uint32_t j = batch & ((1u << lg_ns) - 1u);
+        if (q != have_q) { o = philox4x32_10(q, tile_id, u, rg, p.k0, p.k1); have_q = q; }
+        uint32_t v;
+        if (w16) {
+            const uint32_t word = (j >> 1) == 0 ? o.x : (j >> 1) == 1 ? o.y : (j >> 1) == 2 ? o.z : o.w;
+            v = (word >> (16u * (j & 1u))) & 0xFFFFu;
+        } else {
+            v = j == 0 ? o.x : j == 1 ? o.y : j == 2 ? o.z : o.w;
+        }
+        const uint32_t dx = v & (Se - 1), dy = (v >> lgSe) & (Se - 1);
+        const uint32_t x = (x0 + dx) & Lm, y = (y0 + dy) & Lm;
+        int32_t *row = h + (size_t)y * L;
+        const int32_t c = row[x] + 1;
+        const int32_t l = row[(x - 1) & Lm], r = row[(x + 1) & Lm];
+        const int32_t up = h[(size_t)((y - 1) & Lm) * L + x], dn = h[(size_t)((y + 1) & Lm) * L + x];
+        const bool ok = abs(c - l) <= N && abs(c - r) <= N && abs(c - up) <= N && abs(c - dn) <= N;
+        if (ok) { row[x] = c; ++nacc; }
+    }
+    return nacc;
+}
+
+__global__ void __launch_bounds__(128) simple_dt_kernel(Params p, uint32_t u, uint32_t colour)
+{
+    const uint32_t T = p.L >> p.lgS, half = T >> 1, ntile = half * half;
+    const uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= p.R * ntile) return;
+    const uint32_t rl = idx / ntile, n = idx - rl * ntile;
+    const uint32_t i = n % half, j = n / half;
+    const uint32_t I = 2 * i + (colour & 1u), J = 2 * j + (colour >> 1);
+    const uint32_t rg = p.first_real + rl;
+    uint32_t ox, oy;
+    draw_origin(p, u, rg, ox, oy);
+    const uint32_t x0 = (ox + I * p.S) & (p.L - 1), y0 = (oy + J * p.S) & (p.L - 1);
+    int32_t *h = p.h + (size_t)rl * p.L * p.L;
+    const uint32_t nacc = simple_run_tile(p, h, rg, u, J * T + I, x0, y0, p.S, p.lgS, ((uint64_t)p.S * p.S) / p.K);
+    if (nacc) atomicAdd(p.accepted + rl, (unsigned long long)nacc);
+}
+
+__global__ void __launch_bounds__(32) simple_rs_kernel(Params p, uint32_t t0, uint32_t mcs)
+{
+    const uint32_t rl = blockIdx.x * blockDim.x + threadIdx.x;
+    if (rl >= p.R) return;
+    int32_t *h = p.h + (size_t)rl * p.L * p.L;
+    unsigned long long nacc = 0;
+    for (uint32_t m = 0; m < mcs; ++m)
+        nacc += simple_run_tile(p, h, p.first_real + rl, t0 + m, 0u, 0u, 0u, p.L, p.lgL, (uint64_t)p.L * p.L);
+    if (nacc) atomicAdd(p.accepted + rl, nacc);
+}
+
+// =============================================================================================
+// WARP engines.  On-chip format (D:4): heights mod 64 (N <= 31 makes every nearest-neighbour
+// difference recoverable), four sites of a 2x2 block per 32-bit word, byte k = (Y&1)*2 + (X&1),
+// low 6 bits = height, top 2 bits of the four bytes = the id of the lane that last wrote the word.
+// =============================================================================================
+constexpr uint32_t HMASK = 0x3F3F3F3Fu;
+
+__device__ __forceinline__ uint32_t lane_tag(uint32_t lane)
+{
+    return ((lane & 3u) << 6) | (((lane >> 2) & 3u) << 14) | (((lane >> 4) & 1u) << 22);
+}
+
+// Geometry of the shared-memory window of one warp.
+//   DT  : window of (S+8) x (S+4) sites whose origin (xa, ya) is 4-/2-aligned in GLOBAL lattice
+//         coordinates; it contains the S x S tile at (offx, offy) and its 1-site halo.
+//   RS  : the whole L x L lattice, periodic.
+template <int LGS, bool WRAP>
+struct Geom {
+    static constexpr uint32_t S = 1u << LGS;
+    static constexpr uint32_t PITCH = WRAP ? (S / 2) : (S + 8) / 2;        // words per block row
+    static constexpr uint32_t ROWS = WRAP ? (S / 2) : (S + 4) / 2;         // block rows
+    static constexpr uint32_t WORDS = PITCH * ROWS;
+    static constexpr uint32_t NBM = S / 2 - 1;                             // block-index mask (RS)
+};
+
+// ---------------------------------------------------------------------------------------------
+// All A attempts of one tile by one warp, exactly as if executed one after another (D:2 step 6).
+//
+// 32 consecutive attempts a0 .. a0+31 are in flight, attempt a on lane a & 31 (the slot layout of
+// D:2 makes each lane the owner of the Philox calls q = 32*c + lane, so it draws its own sites).
+// Window step (D:4):
+//   R  every lane reads the three words holding its 5-point stencil;
+//   D  decides on that snapshot: under Eq. (6) the deposit is rejected iff some neighbour
+//      equals h - N (mod 64);
+//   W  accepting lanes store the updated word, tagged with their lane id;
+//   V  every lane re-reads its three words.  A lane is DIRTY if a stencil site changed under it or
+//      its own store is not what the word now holds -- i.e. another accepting lane of this window
+//      wrote the same or an adjacent site (or the same word).
+//   C  f = lowest dirty rank (rank = position in the window); ranks < f are final.  Lanes >= f
+//      whose store survived undo it; all of them are retried in the next window, which starts at
+//      a0 + f.  Rank 0 depends on nothing, so if it is dirty it is re-applied alone (f = 1).
+// Two attempts interact only through equal or adjacent sites, so the committed prefix is exactly
+// the sequential result.  Returns the number of accepted deposits of this lane.
+// ---------------------------------------------------------------------------------------------
+template <int LGS, bool WRAP>
+__device__ __forceinline__ uint32_t warp_run_attempts(uint32_t *sm, uint32_t A, uint32_t tile_id, uint32_t u,
+                                                      uint32_t rg, uint32_t k0, uint32_t k1, uint32_t offx,
+                                                      uint32_t offy, uint32_t N, uint32_t lane)
+{
+    using G = Geom<LGS, WRAP>;
+    constexpr uint32_t S = G::S, PITCH = G::PITCH;
+    const uint32_t FULL = 0xFFFFFFFFu;
+    const uint32_t TAG = lane_tag(lane);
+    const uint32_t nbatch = (A + 31u) >> 5;
+    const uint32_t ncalls = (nbatch + 7u) >> 3;
+    uint32_t my_acc = 0;
+    uint32_t a0 = 0;
+    uint4 cur, nxt = philox4x32_10(lane, tile_id, u, rg, k0, k1);
+    for (uint32_t call = 0; call < ncalls; ++call) {
+        cur = nxt;
+        if (call + 1 < ncalls) nxt = philox4x32_10(32u * (call + 1) + lane, tile_id, u, rg, k0, k1);
+        for (uint32_t j0 = 0; j0 < 8; ++j0) {
+            const uint32_t batch = call * 8 + j0;
+            if (batch >= nbatch) break;
+            // 16-bit slots j0 (this batch) and j0 + 1 (the next batch: lanes that are already past
+            // the batch boundary); both are warp-uniform choices of register, hoisted per batch.
+            const uint32_t wA = (j0 & 4) ? ((j0 & 2) ? cur.w : cur.z) : ((j0 & 2) ? cur.y : cur.x);
+            const uint32_t vA = (wA >> (16u * (j0 & 1u))) & 0xFFFFu;
+            const uint32_t j1 = j0 + 1;
+            const uint32_t wB = (j1 & 8) ? nxt.x : (j1 & 4) ? ((j1 & 2) ? cur.w : cur.z) : ((j1 & 2) ? cur.y : cur.x);
+            const uint32_t vB = (wB >> (16u * (j1 & 1u))) & 0xFFFFu;
+            const uint32_t batch_end = min((batch + 1u) << 5, A);
+            while (a0 < batch_end) {
+                const uint32_t s = a0 & 31u;
+                const uint32_t rank = (lane - s) & 31u;
+                const bool valid = a0 + rank < A;
+                const uint32_t v = (lane >= s) ? vA : vB;
+                const uint32_t X = (v & (S - 1)) + offx;
+                const uint32_t Y = ((v >> LGS) & (S - 1)) + offy;
+                const uint32_t px = X & 1u, py = Y & 1u, k = px | (py << 1);
+                const uint32_t bx = X >> 1, by = Y >> 1;
+                const uint32_t wC = by * PITCH + bx;
+                uint32_t wH, wV;
+                if (WRAP) {
+                    wH = by * PITCH + ((bx - 1u + 2u * px) & G::NBM);
+                    wV = ((by - 1u + 2u * py) & G::NBM) * PITCH + bx;
+                } else {
+                    wH = wC - 1u + 2u * px;
+                    wV = py ? wC + PITCH : wC - PITCH;
+                }
+                // R
+                const uint32_t C = sm[wC], H = sm[wH], V = sm[wV];
+                // D: P = [C(k^1), C(k^2), H(k^1), C(k)], Q = [.., .., .., V(k^2)] -> 4 neighbours
+                const uint32_t kk = k * 0x1111u;
+                const uint32_t P = __byte_perm(C, H, kk ^ 0x0521u);
+                const uint32_t Q = __byte_perm(P, V, (k << 12) ^ 0x6210u);
+                const uint32_t t = ((P >> 24) - N) & 0x3Fu;
+                const uint32_t vv = (Q & HMASK) ^ (t * 0x01010101u);
+                const uint32_t z = (vv - 0x01010101u) & ~vv & 0x80808080u;   // a zero byte <=> nb == h - N
+                const bool acc = valid && (z == 0u);
+                const uint32_t W = (((C & HMASK) + (1u << (8u * k))) & HMASK) | TAG;
+                __syncwarp();
+                // W
+                if (acc) sm[wC] = W;
+                __syncwarp();
+                // V
+                const uint32_t C2 = sm[wC], H2 = sm[wH], V2 = sm[wV];
+                const uint32_t selD = ((k ^ 1u) | ((k ^ 6u) << 4)) * 0x0101u;
+                const uint32_t dHV = __byte_perm(H2 ^ H, V2 ^ V, selD) & HMASK;
+                const bool own_ok = acc ? (C2 == W) : (((C2 ^ C) & HMASK) == 0u);
+                const bool dirty = valid && (!own_ok || dHV != 0u);
+                // C
+                uint32_t f = __reduce_min_sync(FULL, dirty ? rank : 32u);
+                if (f < 32u) {
+                    // slow path: some lane is dirty
+                    if (f == 0u) f = 1u;
+                    const bool committed = rank < f;
+                    if (acc && !committed && C2 == W) sm[wC] = C;      // undo a surviving store
+                    __syncwarp();
+                    if (acc && rank == 0u) sm[wC] = W;                 // rank 0 always stands
+                    __syncwarp();
+                    my_acc += (acc && committed) ? 1u : 0u;
+                } else {
+                    f = min(32u, A - a0);
+                    my_acc += acc ? 1u : 0u;
+                }
+                a0 += f;
+            }
+        }
+    }
+    return my_acc;
+}
+
+__device__ __forceinline__ int32_t sext6(uint32_t d)
+{
+    return ((int32_t)(d << 26)) >> 26;
+}
+
+template <int LGS, bool WRAP>
+__device__ __forceinline__ uint32_t sm_height(const uint32_t *sm, uint32_t X, uint32_t Y)
+{
+    using G = Geom<LGS, WRAP>;
+    const uint8_t *b = reinterpret_cast<const uint8_t *>(sm);
+    return b[((Y >> 1) * G::PITCH + (X >> 1)) * 4u + ((Y & 1u) << 1) + (X & 1u)] & 0x3Fu;
+}
+
+// ---------------------------------------------------------------------------------------------
+// warp_dt: one colour pass of one sub-sweep, one warp per active tile (D:2 steps 4-6, D:4).
+// ---------------------------------------------------------------------------------------------
+template <int LGS>
+__global__ void __launch_bounds__(WARP_DT_WARPS * 32) warp_dt_kernel(Params p, uint32_t u, uint32_t colour)
+{
+    using G = Geom<LGS, false>;
+    constexpr uint32_t S = G::S, PITCH = G::PITCH;
+    constexpr uint32_t NCH = (S + 8) / 4;            // int4 chunks per window row
+    constexpr uint32_t NROW = S + 2;                 // window rows actually needed
+    extern __shared__ __align__(16) uint32_t smem[];
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    uint32_t *sm = smem + warp * G::WORDS;
+
+    const uint32_t L = p.L, Lm = L - 1;
+    const uint32_t T = L >> LGS, half = T >> 1, ntile = half * half;
+    const uint32_t idx = blockIdx.x * WARP_DT_WARPS + warp;
+    if (idx >= p.R * ntile) return;
+    const uint32_t rl = idx / ntile, n = idx - rl * ntile;
+    const uint32_t ti = n % half, tj = n / half;
+    const uint32_t I = 2 * ti + (colour & 1u), J = 2 * tj + (colour >> 1);
+    const uint32_t rg = p.first_real + rl;
+    uint32_t ox, oy;
+    draw_origin(p, u, rg, ox, oy);
+    const uint32_t x0 = (ox + I * S) & Lm, y0 = (oy + J * S) & Lm;
+    const uint32_t offx = ((x0 - 1u) & 3u) + 1u, offy = ((y0 - 1u) & 1u) + 1u;
+    const uint32_t xa = (x0 - offx) & Lm;            // multiple of 4
+    int32_t *h = p.h + (size_t)rl * L * L;
+
+    // ---- stage: rows y0-1 .. y0+S, columns xa .. xa+S+7, low 6 bits of each height ----------
+    {
+        uint16_t *sm16 = reinterpret_cast<uint16_t *>(sm);
+#pragma unroll 4
+        for (uint32_t it = lane; it < NROW * NCH; it += 32u) {
+            const uint32_t yr = it / NCH, c = it - yr * NCH;
+            const uint32_t Y = offy - 1u + yr;
+            const uint32_t gx = (xa + 4u * c) & Lm, gy = (y0 - 1u + yr) & Lm;
+            const int4 q = *reinterpret_cast<const int4 *>(h + (size_t)gy * L + gx);
+            const uint32_t lo = ((uint32_t)q.x & 0x3Fu) | (((uint32_t)q.y & 0x3Fu) << 8);
+            const uint32_t hi = ((uint32_t)q.z & 0x3Fu) | (((uint32_t)q.w & 0x3Fu) << 8);
+            const uint32_t w16 = (((Y >> 1) * PITCH + 2u * c) << 1) + (Y & 1u);   // uint16 index
+            sm16[w16] = (uint16_t)lo;
+            sm16[w16 + 2u] = (uint16_t)hi;
+        }
+    }
+    __syncwarp();
+
+    const uint32_t A = (S * S) / p.K;
+    const uint32_t my_acc = warp_run_attempts<LGS, false>(sm, A, J * T + I, u, rg, p.k0, p.k1, offx, offy, p.N, lane);
+    __syncwarp();
+
+    // ---- write back: int32 heights rebuilt column by column from the frozen halo row ----------
+    // h(x, y) = h(x, y-1) + sext6(b(x, y) - b(x, y-1)): adjacent heights differ by <= N <= 31.
+#pragma unroll 1
+    for (uint32_t cx = lane; cx < S; cx += 32u) {
+        const uint32_t X = offx + cx, gx = (x0 + cx) & Lm;
+        int32_t hv = h[(size_t)((y0 - 1u) & Lm) * L + gx];
+        uint32_t bprev = sm_height<LGS, false>(sm, X, offy - 1u);
+#pragma unroll 8
+        for (uint32_t dy = 0; dy < S; ++dy) {
+            const uint32_t b = sm_height<LGS, false>(sm, X, offy + dy);
+            hv += sext6(b - bprev);
+            bprev = b;
+            h[(size_t)((y0 + dy) & Lm) * L + gx] = hv;
+        }
+    }
+    const uint32_t tot = __reduce_add_sync(0xFFFFFFFFu, my_acc);
+    if (lane == 0 && tot) atomicAdd(p.accepted + rl, (unsigned long long)tot);
+}
+
+// ---------------------------------------------------------------------------------------------
+// warp_rs: RS mode (2S > L): the schedule is serial random-sequential deposition on the whole
+// lattice (D:2 step 3).  One warp per realization; the lattice is staged once, all `mcs` sweeps
+// run on chip, and the int32 heights are rebuilt at the end from differences plus the exact
+// identity  sum h(end) = sum h(start) + accepted.
+// ---------------------------------------------------------------------------------------------
+template <int LGL>
+__global__ void __launch_bounds__(WARP_RS_WARPS * 32) warp_rs_kernel(Params p, uint32_t t0, uint32_t mcs)
+{
+    using G = Geom<LGL, true>;
+    constexpr uint32_t L = G::S, PITCH = G::PITCH;
+    extern __shared__ __align__(16) uint32_t smem[];
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    uint32_t *sm = smem + warp * G::WORDS;
+    const uint32_t rl = blockIdx.x * WARP_RS_WARPS + warp;
+    if (rl >= p.R) return;
+    const uint32_t rg = p.first_real + rl;
+    int32_t *h = p.h + (size_t)rl * L * L;
+    const uint32_t FULL = 0xFFFFFFFFu;
+
+    // ---- stage the whole lattice; S1 = sum of the int32 heights (exact, int64) ----------------
+    long long s1 = 0;
+    {
+        uint16_t *sm16 = reinterpret_cast<uint16_t *>(sm);
+        constexpr uint32_t NCH = L / 4;
+        for (uint32_t it = lane; it < L * NCH; it += 32u) {
+            const uint32_t Y = it / NCH, c = it - Y * NCH;
+            const int4 q = *reinterpret_cast<const int4 *>(h + (size_t)Y * L + 4u * c);
+            s1 += (long long)q.x + q.y + q.z + q.w;
+            const uint32_t lo = ((uint32_t)q.x & 0x3Fu) | (((uint32_t)q.y & 0x3Fu) << 8);
+            const uint32_t hi = ((uint32_t)q.z & 0x3Fu) | (((uint32_t)q.w & 0x3Fu) << 8);
+            const uint32_t w16 = (((Y >> 1) * PITCH + 2u * c) << 1) + (Y & 1u);
+            sm16[w16] = (uint16_t)lo;
+            sm16[w16 + 2u] = (uint16_t)hi;
+        }
+    }
+    __syncwarp();
+
+    unsigned long long my_acc = 0;
+    for (uint32_t m = 0; m < mcs; ++m)
+        my_acc += warp_run_attempts<LGL, true>(sm, L * L, 0u, t0 + m, rg, p.k0, p.k1, 0u, 0u, p.N, lane);
+    __syncwarp();
+
+    unsigned long long tot = my_acc;
+    for (int o = 16; o; o >>= 1) {
+        tot += __shfl_xor_sync(FULL, tot, o);
+        s1 += __shfl_xor_sync(FULL, s1, o);
+    }
+    if (tot == 0ull) return;                       // nothing deposited: global heights are current
+
+    // ---- rebuild: rel(x, y) = h(x, y) - h(0, 0) by difference chains --------------------------
+    // row 0 by a warp scan along x, then every column downwards.
+    constexpr uint32_t NG = (L + 31) / 32;          // column groups per lane
+    int32_t rel0[NG];
+    int32_t carry = 0;
+#pragma unroll
+    for (uint32_t g = 0; g < NG; ++g) {
+        const uint32_t X = g * 32u + lane;
+        int32_t d = 0;
+        if (X < L && X > 0) d = sext6(sm_height<LGL, true>(sm, X, 0) - sm_height<LGL, true>(sm, X - 1u, 0));
+        for (int o = 1; o < 32; o <<= 1) {
+            const int32_t n = __shfl_up_sync(FULL, d, o);
+            if ((int)lane >= o) d += n;
+        }
+        rel0[g] = d + carry;
+        carry = __shfl_sync(FULL, rel0[g], 31);
+    }
+    long long srel = 0;
+#pragma unroll
+    for (uint32_t g = 0; g < NG; ++g) {
+        const uint32_t X = g * 32u + lane;
+        if (X < L) {
+            int32_t rv = rel0[g];
+            uint32_t bprev = sm_height<LGL, true>(sm, X, 0);
+            srel += rv;
+            for (uint32_t Y = 1; Y < L; ++Y) {
+                const uint32_t b = sm_height<LGL, true>(sm, X, Y);
+                rv += sext6(b - bprev);
+                bprev = b;
+                srel += rv;
+            }
+        }
+    }
+    for (int o = 16; o; o >>= 1) srel += __shfl_xor_sync(FULL, srel, o);
+    // L^2 * h00 + srel = s1 + accepted
+    const long long num = s1 + (long long)tot - srel;
+    const long long h00 = num >> (2 * LGL);
+    if ((h00 << (2 * LGL)) != num) { if (lane == 0) atomicOr(p.err, ERR_RECONSTRUCT); return; }
+#pragma unroll
+    for (uint32_t g = 0; g < NG; ++g) {
+        const uint32_t X = g * 32u + lane;
+        if (X < L) {
+            int32_t hv = (int32_t)h00 + rel0[g];
+            uint32_t bprev = sm_height<LGL, true>(sm, X, 0);
+            h[X] = hv;
+            for (uint32_t Y = 1; Y < L; ++Y) {
+                const uint32_t b = sm_height<LGL, true>(sm, X, Y);
+                hv += sext6(b - bprev);
+                bprev = b;
+                h[(size_t)Y * L + X] = hv;
+            }
+        }
+    }
+    if (lane == 0) atomicAdd(p.accepted + rl, tot);
+}
+
+// =============================================================================================
+// Host-side launchers
+// =============================================================================================
+size_t warp_dt_smem(uint32_t lgS)
+{
+    const uint32_t S = 1u << lgS;
+    return (size_t)WARP_DT_WARPS * ((S + 8) / 2) * ((S + 4) / 2) * 4;
+}
+size_t warp_rs_smem(uint32_t lgL)
+{
+    const uint32_t L = 1u << lgL;
+    return (size_t)WARP_RS_WARPS * (L / 2) * (L / 2) * 4;
+}
+
+template <int LGS>
+static cudaError_t launch_warp_dt_t(const Params &p, uint32_t u, uint32_t colour, uint32_t blocks, cudaStream_t st,
+                                    bool configure)
+{
+    const size_t sm = warp_dt_smem(LGS);
+    if (configure) return cudaFuncSetAttribute(warp_dt_kernel<LGS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    warp_dt_kernel<LGS><<<blocks, WARP_DT_WARPS * 32, sm, st>>>(p, u, colour);
+    return cudaGetLastError();
+}
+
+static cudaError_t dispatch_warp_dt(const Params &p, uint32_t u, uint32_t colour, uint32_t blocks, cudaStream_t st,
+                                    bool configure)
+{
+    switch (p.lgS) {
+        case 3: return launch_warp_dt_t<3>(p, u, colour, blocks, st, configure);
+        case 4: return launch_warp_dt_t<4>(p, u, colour, blocks, st, configure);
+        case 5: return launch_warp_dt_t<5>(p, u, colour, blocks, st, configure);
+        case 6: return launch_warp_dt_t<6>(p, u, colour, blocks, st, configure);
+        case 7: return launch_warp_dt_t<7>(p, u, colour, blocks, st, configure);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+template <int LGL>
+static cudaError_t launch_warp_rs_t(const Params &p, uint32_t t0, uint32_t mcs, uint32_t blocks, cudaStream_t st,
+                                    bool configure)
+{
+    const size_t sm = warp_rs_smem(LGL);
+    if (configure) return cudaFuncSetAttribute(warp_rs_kernel<LGL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    warp_rs_kernel<LGL><<<blocks, WARP_RS_WARPS * 32, sm, st>>>(p, t0, mcs);
+    return cudaGetLastError();
+}
+
+static cudaError_t dispatch_warp_rs(const Params &p, uint32_t t0, uint32_t mcs, uint32_t blocks, cudaStream_t st,
+                                    bool configure)
+{
+    switch (p.lgL) {
+        case 2: return launch_warp_rs_t<2>(p, t0, mcs, blocks, st, configure);
+        case 3: return launch_warp_rs_t<3>(p, t0, mcs, blocks, st, configure);
+        case 4: return launch_warp_rs_t<4>(p, t0, mcs, blocks, st, configure);
+        case 5: return launch_warp_rs_t<5>(p, t0, mcs, blocks, st, configure);
+        case 6: return launch_warp_rs_t<6>(p, t0, mcs, blocks, st, configure);
+        case 7: return launch_warp_rs_t<7>(p, t0, mcs, blocks, st, configure);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+cudaError_t configure_engine(const Params &p, uint32_t engine, bool mode_dt)
+{
+    if (engine == ENGINE_WARP && mode_dt) return dispatch_warp_dt(p, 0, 0, 0, nullptr, true);
+    if (engine == ENGINE_ONCHIP && !mode_dt) return dispatch_warp_rs(p, 0, 0, 0, nullptr, true);
+    return cudaSuccess;
+}
+
+uint32_t engine_blocks(const Params &p, uint32_t engine, bool mode_dt)
+{
+    const uint32_t T = p.L >> p.lgS, half = T >> 1;
+    const uint64_t tiles = mode_dt ? (uint64_t)p.R * half * half : p.R;
+    if (engine == ENGINE_WARP) return (uint32_t)((tiles + WARP_DT_WARPS - 1) / WARP_DT_WARPS);
+    if (engine == ENGINE_ONCHIP) return (uint32_t)((tiles + WARP_RS_WARPS - 1) / WARP_RS_WARPS);
+    return (uint32_t)((tiles + (mode_dt ? 127 : 31)) / (mode_dt ? 128 : 32));
+}
+
+// One colour pass of sub-sweep u (DT mode).
+cudaError_t launch_dt_pass(const Params &p, uint32_t engine, uint32_t u, uint32_t colour, cudaStream_t st)
+{
+    const uint32_t blocks = engine_blocks(p, engine, true);
+    if (engine == ENGINE_WARP) return dispatch_warp_dt(p, u, colour, blocks, st, false);
+    simple_dt_kernel<<<blocks, 128, 0, st>>>(p, u, colour);
+    return cudaGetLastError();
+}
+
+// `mcs` whole sweeps starting at sweep counter t0 (RS mode).
+cudaError_t launch_rs_sweeps(const Params &p, uint32_t engine, uint32_t t0, uint32_t mcs, cudaStream_t st)
+{
+    const uint32_t blocks = engine_blocks(p, engine, false);
+    if (engine == ENGINE_ONCHIP) return dispatch_warp_rs(p, t0, mcs, blocks, st, false);
+    simple_rs_kernel<<<blocks, 32, 0, st>>>(p, t0, mcs);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------
+// Philox test hook (rsos_philox): the same device function on n (counter, key) pairs.
+// ---------------------------------------------------------------------------------------------
+__global__ void philox_kernel(const uint32_t *ctr, const uint32_t *key, uint32_t *out, uint32_t n)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint4 o = philox4x32_10(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3], key[2 * i], key[2 * i + 1]);
+    out[4 * i] = o.x; out[4 * i + 1] = o.y; out[4 * i + 2] = o.z; out[4 * i + 3] = o.w;
+}
+
+cudaError_t launch_philox(const uint32_t *d_ctr, const uint32_t *d_key, uint32_t *d_out, uint32_t n, cudaStream_t st)
+{
+    philox_kernel<<<(n + 255) / 256, 256, 0, st>>>(d_ctr, d_key, d_out, n);
+    return cudaGetLastError();
+}
+
+}  // namespace rsos

@@ -1,0 +1,36 @@
+"""Seeded synthetic workloads (BASELINE.json configs C1..C5) and measurement-time schedules.
+
+Shared by tests, bench.py and the oracle harness.  Holds NONE of the method's arithmetic: an RSOS
+workload is fully described by (L, N, R, seed, tile S, sub-sweeps K, MCS); the lattice starts flat
+ and every random number is drawn inside the implementations from Philox.
+"""
+import math
+
+# name -> dict(L, N, R, mcs, seed, tile, subsweeps); lists mean "one run per entry"
+CONFIGS = {
+    "C1": dict(L=32, N=1, R=128, mcs=100, seed=1, tile=64, subsweeps=1),
+    "C2": dict(L=1024, N=1, R=128, mcs=10_000, seed=1, tile=64, subsweeps=1),      # seeds 1..4
+    "C3": dict(L=2048, N=1, R=64, mcs=5_000, seed=1, tile=64, subsweeps=1),        # N in 1..4
+    "C4": dict(L=32768, N=1, R=1, mcs=2_000, seed=1, tile=64, subsweeps=1),
+    "C5": dict(L=64, N=1, R=4096, mcs=15_521, seed=1, tile=64, subsweeps=4),       # L in 64..512, N in 1,2
+}
+
+
+def c5_realizations(L):
+    """BASELINE.json C5: 4096 realizations at L = 64, scaled as 1/L^2 (R * L^2 = 2^24)."""
+    return (1 << 24) // (L * L)
+
+
+def c5_mcs(L):
+    """BASELINE.json C5: run to t = 20 * L^1.6 MCS."""
+    return int(math.ceil(20.0 * L ** 1.6))
+
+
+def log_spaced_times(t_max, n=64):
+    """sorted(set(round(t_max^(j/(n-1))))) for j = 0..n-1: the `n log-spaced times` of C2-C4."""
+    return sorted({int(round(t_max ** (j / (n - 1)))) for j in range(n)})
+
+
+def attempts(L, R, mcs):
+    """1 MCS = L*L attempts per realization (reading Q4)."""
+    return int(L) * int(L) * int(R) * int(mcs)

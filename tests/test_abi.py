@@ -1,0 +1,82 @@
+"""CPU-side checks of the boundary: librsos.so builds (nvcc cross-compiles for sm_100a), loads, and
+exports exactly the entry points include/rsos.h declares; without a GPU every call fails loudly
+(no CPU fallback); the product package never imports the oracle."""
+import ctypes
+import os
+import re
+import subprocess
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib_path():
+    from paper_1605_02620_b200 import build
+    return build.build()
+
+
+def header_functions():
+    src = open(os.path.join(ROOT, "include", "rsos.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(rsos_[a-z_]+)\s*\(", src)))
+
+
+def test_header_declares_the_north_star_calls():
+    names = header_functions()
+    for need in ("rsos_init", "rsos_advance", "rsos_width"):
+        assert need in names
+
+
+def test_library_exports_every_declared_symbol(lib_path):
+    import paper_1605_02620_b200 as m
+    names = header_functions()
+    assert sorted(m.SYMBOLS) == names
+    out = subprocess.check_output(["nm", "-D", "--defined-only", lib_path], text=True)
+    exported = sorted(set(re.findall(r" T (rsos_[a-z_]+)$", out, flags=re.M)))
+    assert exported == names
+    lib = ctypes.CDLL(lib_path)
+    for n in names:
+        assert getattr(lib, n) is not None
+
+
+def test_library_is_sm100a_only(lib_path):
+    out = subprocess.check_output(["cuobjdump", "-lelf", lib_path], text=True)
+    archs = set(re.findall(r"sm_(\d+a?)", out))
+    assert archs == {"100a"}, archs
+
+
+def test_no_cpu_fallback_without_a_device():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    import paper_1605_02620_b200 as m
+    with pytest.raises(m.RsosError) as e:
+        m.Rsos(32, 1, 4, 1)
+    assert e.value.code == -4
+    with pytest.raises(m.RsosError):
+        m.philox([[0, 0, 0, 0]], [[0, 0]])
+
+
+def test_argument_errors_need_no_device(lib_path):
+    import paper_1605_02620_b200 as m
+    for args, kw, code in [((48, 1, 1, 1), {}, -1), ((64, 0, 1, 1), {}, -1), ((64, 1, 0, 1), {}, -1),
+                           ((128, 1, 1, 1), dict(tile=24), -1), ((64, 1, 1, 1), dict(engine=m.ENGINE_WARP), -5),
+                           ((256, 1, 1, 1), dict(engine=m.ENGINE_ONCHIP), -5), ((128, 32, 1, 1), dict(engine=m.ENGINE_WARP), -5)]:
+        with pytest.raises(m.RsosError) as e:
+            m.Rsos(*args, **kw)
+        assert e.value.code == code, (args, kw)
+
+
+def test_product_never_touches_the_oracle():
+    pkg = os.path.join(ROOT, "paper_1605_02620_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle|rsos_oracle|#include\s+\".*oracle", text, flags=re.M), f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            text = open(os.path.join(ROOT, "oracle", f)).read()
+            assert not re.search(r"^\s*(from|import)\s+paper_1605_02620_b200|#include\s+\".*csrc", text, flags=re.M), f

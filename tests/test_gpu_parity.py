@@ -1,0 +1,226 @@
+"""GPU parity (run on the B200 with -m gpu): the CUDA path behind the C ABI against the CPU oracle.
+
+Integer work, so the bar is bit-exact: heights element by element, and (S1, S2, accepted) exactly
+(BASELINE.json north_star).  Both sides execute the seeded schedule of DESIGN.md section 2 on the
+same (L, N, R, seed, S, K); no expected value comes from the CUDA path.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def rsos():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1605_02620_b200 import build
+    build.build()
+    import paper_1605_02620_b200 as m
+    return m
+
+
+def compare(g, o, what=""):
+    gs1, gs2, gacc = g.sums()
+    os1, os2, oacc = o.sums()
+    assert (gs1 == os1).all(), what + " S1"
+    assert (gs2 == os2).all(), what + " S2"
+    assert (gacc == oacc).all(), what + " accepted"
+    hg, ho = g.heights(), o.heights()
+    bad = np.argwhere(hg != ho)
+    assert bad.size == 0, "%s heights differ at %d sites, first %s" % (what, len(bad), bad[:5].tolist())
+    gw, gh = g.width()
+    ow, oh = o.width()
+    assert (gw == ow).all() and (gh == oh).all(), what + " W2/hmean doubles"
+
+
+def test_philox_device_equals_oracle(rsos, oracle_mod):
+    rng = np.random.default_rng(3)
+    n = 20000
+    ctr = rng.integers(0, 2 ** 32, size=(n, 4), dtype=np.uint64).astype(np.uint32)
+    key = rng.integers(0, 2 ** 32, size=(n, 2), dtype=np.uint64).astype(np.uint32)
+    ctr[0] = 0; key[0] = 0
+    ctr[1] = 0xFFFFFFFF; key[1] = 0xFFFFFFFF
+    out = rsos.philox(ctr, key)
+    assert out[0].tolist() == [0x6627e8d5, 0xe169c58d, 0xbc57ac4c, 0x9b00dbd8]      # tests/golden/philox_kat.txt
+    assert out[1].tolist() == [0x408f276d, 0x41c83b0e, 0xa20bc7c6, 0x6d5451fd]
+    for i in range(0, n, 7):
+        assert (out[i] == oracle_mod.philox(ctr[i], key[i])).all()
+
+
+@pytest.mark.parametrize("engine", ["onchip", "simple"])
+def test_c1_full_config_every_mcs(rsos, oracle_mod, engine):
+    """BASELINE.json configs[0]: L=32, N=1, R=128, 100 MCS, seed 1, sums at every MCS (tier A)."""
+    eng = {"onchip": rsos.ENGINE_ONCHIP, "simple": rsos.ENGINE_SIMPLE}[engine]
+    g = rsos.Rsos(32, 1, 128, 1, engine=eng)
+    o = oracle_mod.Oracle(32, 1, 128, 1)
+    assert g.info()["mode"] == "RS" and o.mode == "RS"
+    for t in range(100):
+        g.advance(1)
+        o.advance(1)
+        gs, os_ = g.sums(), o.sums()
+        assert all((a == b).all() for a, b in zip(gs, os_)), "t=%d" % (t + 1)
+    compare(g, o, "C1 " + engine)
+    g.close()
+
+
+@pytest.mark.parametrize("L,N,R,S,K,mcs,seed", [
+    (128, 1, 3, 64, 1, 6, 1),        # smallest DT lattice at the default tile: T = 2, one tile per colour
+    (256, 1, 2, 64, 1, 5, 2),        # several tiles, wrap-around windows
+    (256, 2, 2, 64, 4, 4, 3),        # K = 4 sub-sweeps
+    (256, 4, 1, 64, 1, 4, 4),        # larger slopes (config C3)
+    (512, 3, 1, 64, 2, 3, 5),
+    (128, 1, 2, 32, 4, 5, 6),        # S = 32
+    (64, 2, 3, 16, 1, 5, 7),         # S = 16
+    (64, 1, 2, 8, 2, 5, 8),          # S = 8, A = 32 attempts per tile
+    (256, 1, 1, 128, 1, 3, 9),       # S = 128
+    (128, 31, 1, 64, 1, 3, 10),      # largest N of the 6-bit on-chip format
+    (128, 1, 1, 64, 128, 2, 11),     # A = 32: a single window per tile
+])
+def test_dt_warp_engine_equals_oracle(rsos, oracle_mod, L, N, R, S, K, mcs, seed):
+    g = rsos.Rsos(L, N, R, seed, tile=S, subsweeps=K, engine=rsos.ENGINE_WARP)
+    o = oracle_mod.Oracle(L, N, R, seed, tile=S, subsweeps=K)
+    assert g.info()["mode"] == "DT" and o.mode == "DT"
+    for step in range(mcs):
+        g.advance(1)
+        o.advance(1)
+        compare(g, o, "DT warp L=%d N=%d S=%d K=%d t=%d" % (L, N, S, K, step + 1))
+    g.close()
+
+
+@pytest.mark.parametrize("L,N,R,S,K,mcs", [(128, 1, 2, 64, 1, 3), (128, 2, 2, 16, 4, 3), (1024, 1, 1, 512, 1, 1),
+                                           (128, 40, 1, 64, 1, 2)])
+def test_dt_simple_engine_equals_oracle(rsos, oracle_mod, L, N, R, S, K, mcs):
+    g = rsos.Rsos(L, N, R, 21, tile=S, subsweeps=K, engine=rsos.ENGINE_SIMPLE if N <= 31 else rsos.ENGINE_AUTO)
+    assert g.info()["engine"] == "simple"
+    o = oracle_mod.Oracle(L, N, R, 21, tile=S, subsweeps=K)
+    g.advance(mcs)
+    o.advance(mcs)
+    compare(g, o, "DT simple")
+    g.close()
+
+
+@pytest.mark.parametrize("L,N,R,mcs", [(4, 1, 5, 30), (8, 2, 33, 20), (16, 1, 7, 20), (64, 1, 9, 12), (64, 3, 4, 12),
+                                       (128, 1, 3, 5), (32, 31, 2, 40)])
+def test_rs_onchip_engine_equals_oracle(rsos, oracle_mod, L, N, R, mcs):
+    """RS mode (2S > L): serial random-sequential dynamics with the whole lattice on chip."""
+    g = rsos.Rsos(L, N, R, 5, tile=128, engine=rsos.ENGINE_ONCHIP)
+    o = oracle_mod.Oracle(L, N, R, 5, tile=128)
+    assert g.info()["mode"] == "RS" and o.mode == "RS"
+    g.advance(3)                      # several sweeps inside one launch ...
+    g.advance(mcs - 3)                # ... and a second call continuing from the stored heights
+    o.advance(mcs)
+    compare(g, o, "RS onchip L=%d N=%d" % (L, N))
+    g.close()
+
+
+def test_rs_simple_large_lattice_32bit_slots(rsos, oracle_mod):
+    """RS with L = 512: 2 lg L > 16 selects the 32-bit slot layout (4 slots per Philox call)."""
+    g = rsos.Rsos(512, 1, 2, 9, tile=512)
+    assert g.info() ["engine"] == "simple" and g.info()["mode"] == "RS"
+    o = oracle_mod.Oracle(512, 1, 2, 9, tile=512)
+    g.advance(1)
+    o.advance(1)
+    compare(g, o, "RS simple L=512")
+    g.close()
+
+
+def test_first_real_splits_a_run(rsos, oracle_mod):
+    """Realization r is a pure function of (seed, r, ...): contexts with first_real offsets tile a run."""
+    o = oracle_mod.Oracle(128, 1, 4, 77)
+    o.advance(3)
+    ho = o.heights()
+    for r0 in (0, 1, 3):
+        g = rsos.Rsos(128, 1, 1, 77, first_real=r0)
+        g.advance(3)
+        assert (g.heights()[0] == ho[r0]).all()
+        g.close()
+
+
+def test_snapshot_restart_and_state_roundtrip(rsos, oracle_mod):
+    """rsos_set_state: (heights, t) is the whole state because t sits in the Philox counter."""
+    a = rsos.Rsos(256, 2, 2, 13)
+    a.advance(5)
+    snap = a.heights()
+    _, _, acc = a.sums()
+    a.advance(2)
+    b = rsos.Rsos(256, 2, 2, 13)
+    b.set_state(snap, 5, acc)
+    assert b.t == 5
+    b.advance(2)
+    assert (a.heights() == b.heights()).all()
+    assert all((x == y).all() for x, y in zip(a.sums(), b.sums()))
+    o = oracle_mod.Oracle(256, 2, 2, 13)
+    o.set_state(snap, 5, acc)
+    o.advance(2)
+    compare(b, o, "snapshot")
+    a.close(); b.close()
+
+
+def test_borrowed_torch_buffer_and_stream(rsos, oracle_mod):
+    import torch
+    L, R = 128, 2
+    buf = torch.full((R, L, L), 7, dtype=torch.int32, device="cuda")     # content ignored: flat start
+    st = torch.cuda.Stream()
+    g = rsos.Rsos(L, 1, R, 3, d_heights=buf.data_ptr(), stream=st.cuda_stream)
+    assert g.device_heights() == buf.data_ptr()
+    g.advance(4)
+    o = oracle_mod.Oracle(L, 1, R, 3)
+    o.advance(4)
+    compare(g, o, "borrowed buffer")
+    st.synchronize()
+    assert (buf.cpu().numpy() == o.heights()).all()
+    g.close()
+
+
+def test_invariants_on_device_result(rsos, oracle_mod):
+    """Eq. (6) holds on every bond, heights never decrease, sum h == accepted (pins P1-P3 on the GPU state)."""
+    g = rsos.Rsos(256, 2, 3, 99)
+    prev = g.heights()
+    for _ in range(4):
+        g.advance(2)
+        h = g.heights()
+        assert (h >= prev).all()
+        for r in range(3):
+            assert oracle_mod.violations(h[r], 2) == 0
+        S1, S2, acc = g.sums()
+        assert (S1 == acc).all()
+        assert (S1 == h.reshape(3, -1).astype(np.int64).sum(1)).all()
+        assert (S2 == (h.reshape(3, -1).astype(np.int64) ** 2).sum(1).astype(np.uint64)).all()
+        prev = h
+    g.close()
+
+
+def test_moments_exact(rsos):
+    g = rsos.Rsos(256, 3, 2, 5)
+    g.advance(6)
+    base, M = g.moments()
+    h = g.heights()
+    for r in range(2):
+        d = [int(v) - int(base[r]) for v in h[r].ravel()]
+        assert int(base[r]) == sum(int(v) for v in h[r].ravel()) // (256 * 256)
+        for k in range(4):
+            assert M[r][k] == sum(x ** (k + 1) for x in d)
+    g.close()
+
+
+def test_error_paths(rsos):
+    for args, kw in [((48, 1, 1, 1), {}), ((64, 0, 1, 1), {}), ((64, 1, 0, 1), {}), ((64, 200, 1, 1), {}),
+                     ((128, 1, 1, 1), dict(tile=24)), ((128, 1, 1, 1), dict(tile=8, subsweeps=4)),
+                     ((128, 1, 1, 1), dict(subsweeps=3))]:
+        with pytest.raises(rsos.RsosError) as e:
+            rsos.Rsos(*args, **kw)
+        assert e.value.code == -1
+    with pytest.raises(rsos.RsosError) as e:
+        rsos.Rsos(64, 1, 1, 1, engine=rsos.ENGINE_WARP)          # RS mode cannot use the DT warp engine
+    assert e.value.code == -5
+    g = rsos.Rsos(128, 1, 1, 1, subsweeps=4)
+    with pytest.raises(rsos.RsosError) as e:
+        g.advance(2 ** 30)                                           # (t + mcs) * K reaches 2^32
+    assert e.value.code == -2 and g.t == 0
+    with pytest.raises(rsos.RsosError):
+        g.heights(r0=1, nr=1)
+    g.advance(0)
+    assert g.t == 0
+    g.close()
