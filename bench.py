@@ -1,0 +1,338 @@
+#!/usr/bin/env python
+"""bench.py -- RSOS site-update attempts per second on B200 (BASELINE.json metric), one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2|C4|C1|C5] [--impl reference]
+
+A *step* is one pass of the whole hot path over one
+batch: `mcs_per_step` Monte-Carlo steps of rsos_advance (Philox draws, origin draw, tile staging,
+attempt loop, write-back) followed by one rsos_width (int64 width reduction, result read to host).
+The default workload is BASELINE.json configs[1] (C2: L=1024, N=1, 128 realizations, DT(64,1)); its
+512 MiB of heights exceed the 126 MB L2, so no L2 flush is needed between iterations.
+
+value     whole-job attempts/s with the lattice resident in HBM (device-timed with CUDA events on
+          the stream the kernels run on, barrier + synchronize on both sides, max over ranks).
+e2e       the same metric through the C ABI with HOST buffers: every step restores the lattice from
+          a pinned host snapshot (rsos_set_state, H2D), advances it, and reads W2/<h> back (D2H).
+roofline  dominant kernel (the colour-pass update kernel): algorithmic bytes per launch
+          (8.25 B per attempt) / its average launch duration measured live by
+          rsos_kernel_time (CUDA events on the context's stream), against MEASURED_PEAKS.json.
+cpu_baseline / --impl reference: the CPU oracle as it stands, on a bounded sample of the workload.
+N > 1: replicas only: rank i runs realizations [i*R, (i+1)*R), no collective
+on the data path; scaling is weak.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1605_02620_b200.utils import workloads  # noqa: E402  (no method arithmetic in there)
+
+METRIC = "rsos_site_update_attempts_per_second"
+UNIT = "G attempts/s"
+BYTES_PER_ATTEMPT = 8.25      # 4 B read + 4 B write per site + (4S+4)/S^2 halo re-read, S = 64
+FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="C2", choices=sorted(workloads.CONFIGS))
+    ap.add_argument("--mcs-per-step", type=int, default=0, help="MCS per step (0 = workload default)")
+    ap.add_argument("--engine", default="auto", choices=["auto", "simple", "warp", "onchip", "block"])
+    ap.add_argument("--tile", type=int, default=0)
+    ap.add_argument("--subsweeps", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
+    return ap.parse_args()
+
+
+def workload(args):
+    c = dict(workloads.CONFIGS[args.workload])
+    if args.tile:
+        c["tile"] = args.tile
+    if args.subsweeps:
+        c["subsweeps"] = args.subsweeps
+    # MCS per step: about 20-40 ms of device work per step, far above launch and event overheads
+    default_mcs = {"C1": 1000, "C2": 32, "C3": 16, "C4": 4, "C5": 256}[args.workload]
+    c["mcs_per_step"] = args.mcs_per_step or default_mcs
+    return c
+
+
+def config_dict(args, c, n_gpus):
+    mode = "RS" if 2 * c["tile"] > c["L"] else "DT(%d,%d)" % (c["tile"], c["subsweeps"])
+    return {"workload": "%s: RSOS N=%d, L=%d periodic, %d realizations per GPU, int32 heights, flat start, seed %d"
+                        % (args.workload, c["N"], c["L"], c["R"], c["seed"]),
+            "schedule": mode, "mcs_per_step": c["mcs_per_step"],
+            "step": "rsos_advance(mcs_per_step) + rsos_width",
+            "l2": "state %d MiB per GPU vs 126 MB L2: %s" % (
+                c["R"] * c["L"] ** 2 * 4 >> 20,
+                "inputs larger than L2, no flush" if c["R"] * c["L"] ** 2 * 4 > 2 * 126e6 else "L2/on-chip resident by design"),
+            "parallelism": "replicas x%d (independent realizations, no collective)" % n_gpus}
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe):
+    one `nvidia-smi -lms 50` child, rows kept only between mark() and stop()."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.rows, self.keep, self.proc = [], False, None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            pass
+
+    def run(self):
+        if not self.proc:
+            return
+        for line in self.proc.stdout:
+            f = [x.strip() for x in line.strip().split(",")]
+            if self.keep and len(f) >= 7:
+                self.rows.append(f)
+
+    def mark(self):
+        self.keep = True
+
+    def stop(self):
+        self.keep = False
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except subprocess.TimeoutExpired:
+                self.proc.kill()
+        self.join(timeout=5)
+        rows = []
+        for r in self.rows:
+            try:
+                rows.append((float(r[0]), float(r[1]), float(r[2]), r[3:7]))
+            except ValueError:
+                pass
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"], "samples": 0}
+        sm = sorted(r[0] for r in rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[3][i].lower().startswith("active") for r in rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": rows[0][1], "reasons": reasons,
+                "power_w_max": max(r[2] for r in rows), "samples": len(rows)}
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+# ---------------------------------------------------------------------------------------------
+# CPU oracle legs (the only places bench.py executes oracle/): cpu_baseline and --impl reference
+# ---------------------------------------------------------------------------------------------
+def oracle_sample(c, seconds, steps=1, warmup=0):
+    """Time the oracle as it stands on a bounded sample of workload c: min(R, cores) realizations of
+    the same L, N, S, K, for as many MCS as fit in `seconds` of wall time (calibrated on 1 MCS).
+    Returns (attempts/s, cores, description, ms per step)."""
+    from oracle import rsos_oracle
+    rsos_oracle.build()
+    cores = os.cpu_count() or 1
+    R = min(c["R"], cores)
+    o = rsos_oracle.Oracle(c["L"], c["N"], R, c["seed"], tile=c["tile"], subsweeps=c["subsweeps"])
+    threads = o.threads
+    t0 = time.perf_counter()
+    o.advance(1)
+    dt1 = max(time.perf_counter() - t0, 1e-4)
+    n_total = max(1, steps + warmup)
+    mcs = max(1, min(c["mcs_per_step"] if steps > 1 else 10 ** 9, int(seconds / n_total / dt1)))
+    for _ in range(warmup):
+        o.advance(mcs)
+        o.width()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        o.advance(mcs)
+        o.width()
+    dt = time.perf_counter() - t0
+    o.close()
+    att = workloads.attempts(c["L"], R, mcs) * steps
+    used = min(threads, R) if c["R"] >= threads or 2 * c["tile"] > c["L"] else threads
+    desc = "%d of %d realizations, L=%d, %d MCS per step x %d step(s) + width, OpenMP threads=%d" % (
+        R, c["R"], c["L"], mcs, steps, threads)
+    return att / dt, used, desc, dt / steps * 1e3
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same metric/config; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    c = workload(args)
+    budget = min(150.0, max(20.0, 3.0 * args.cpu_seconds))
+    v, cores, desc, ms = oracle_sample(c, budget, steps=max(1, args.steps), warmup=max(0, args.warmup))
+    line = {"impl": "reference", "metric": METRIC, "value": v / 1e9, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+            "config": config_dict(args, c, args.gpus),
+            "cpu_baseline": {"value": v / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": v / 1e9, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------
+# The B200 arm
+# ---------------------------------------------------------------------------------------------
+def run_b200(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback")
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    from paper_1605_02620_b200 import build as _build
+    if rank == 0:
+        _build.build()
+    barrier()
+    import paper_1605_02620_b200 as pkg
+
+    c = workload(args)
+    L, N, R, mcs = c["L"], c["N"], c["R"], c["mcs_per_step"]
+    engine = {"auto": 0, "simple": 1, "warp": 2, "onchip": 3, "block": 4}[args.engine]
+    stream = torch.cuda.Stream()
+    heights = torch.empty((R, L, L), dtype=torch.int32, device="cuda")      # device memory only: plumbing
+    g = pkg.Rsos(L, N, R, c["seed"], tile=c["tile"], subsweeps=c["subsweeps"], first_real=rank * R, engine=engine,
+                 d_heights=heights.data_ptr(), stream=stream.cuda_stream)
+    info = g.info()
+    att_step = workloads.attempts(L, R, mcs)
+
+    def step():
+        g.advance(mcs)
+        return g.width()
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    barrier()
+
+    # ---- timed region: exactly K steps, CUDA events on the kernels' stream ----------------------
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+        time.sleep(0.3)                                    # let nvidia-smi come up before the timed region
+    g.kernel_time(True)                                    # per-advance CUDA events inside the library
+    launches0 = g.info()["launches"]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    if sampler:
+        sampler.mark()
+    e0.record(stream)
+    for _ in range(args.steps):
+        W2, hmean = step()
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop() if sampler else None
+    upd_ms, upd_launches = g.kernel_time(False)
+    launches = g.info()["launches"] - launches0
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = att_step * args.steps * world / (ms * 1e-3)
+
+    # ---- e2e: host buffers through the C ABI, H2D + D2H inside the timed region -----------------
+    e2e = None
+    if not args.no_e2e:
+        snap = torch.empty((R, L, L), dtype=torch.int32, pin_memory=True)
+        snap_np = snap.numpy()
+        g.heights(out=snap_np)
+        t_snap = g.t
+        _, _, acc = g.sums()
+        for _ in range(2):
+            g.set_state(snap_np, t_snap, acc)
+            step()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            g.set_state(snap_np, t_snap, acc)              # H2D: R*L*L int32 + R int64
+            step()                                         # advance + width (D2H: sums, accepted)
+        barrier()
+        dt = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": att_step * args.steps * world / dt / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": R * L * L * 4 + R * 8, "d2h_bytes_per_step": R * 5 * 8 + 4,
+               "what": "rsos_set_state(pinned host snapshot) + rsos_advance + rsos_width per step, wall clock"}
+        del snap
+
+    if rank != 0:
+        g.close()
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (the update kernel) ------------------------------------
+    hbm, how = peaks()
+    per_launch_att = att_step * args.steps / max(1, upd_launches)
+    avg_ms = upd_ms / max(1, upd_launches)
+    achieved = per_launch_att * BYTES_PER_ATTEMPT / (avg_ms * 1e-3) / 1e9
+    sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
+    alu_bound = info["sm_count"] * 32 * sm_mhz * 1e6 / 6.0          # 6 shared-memory ops / attempt
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": hbm, "unit": "GB/s", "frac": achieved / hbm,
+                "traffic": None, "peak_source": how, "kernel": "update kernel, engine=%s" % info["engine"],
+                "bytes_per_attempt": BYTES_PER_ATTEMPT, "attempts_per_launch": per_launch_att,
+                "avg_launch_ms": avg_ms, "update_share_of_step": upd_ms / ms,
+                "alu_bound_attempts_per_s": alu_bound, "frac_of_alu_bound": (att_step * args.steps / (upd_ms * 1e-3)) / alu_bound,
+                "hbm_bound_attempts_per_s": hbm * 1e9 / BYTES_PER_ATTEMPT}
+
+    cpu = None
+    if not args.no_cpu_baseline and world == 1:
+        v, cores, desc, _ = oracle_sample(c, args.cpu_seconds)
+        cpu = {"value": v / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+
+    line = {"metric": METRIC, "value": value / 1e9, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int32", "data": "synthetic", "config": config_dict(args, c, world),
+            "engine": info, "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+            "cpu_baseline": cpu, "result_check": {"W2_mean": float(np.mean(W2)), "hmean_mean": float(np.mean(hmean)),
+                                                  "t_mcs": int(g.t)}}
+    g.close()
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_b200(args)
+
+
+if __name__ == "__main__":
+    main()
