@@ -48,7 +48,7 @@ def parse():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", default="C2", choices=sorted(workloads.CONFIGS))
     ap.add_argument("--mcs-per-step", type=int, default=0, help="MCS per step (0 = workload default)")
-    ap.add_argument("--engine", default="auto", choices=["auto", "simple", "warp", "onchip", "block"])
+    ap.add_argument("--engine", default="auto", choices=["auto", "simple", "warp", "onchip", "thread"])
     ap.add_argument("--tile", type=int, default=0)
     ap.add_argument("--subsweeps", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -220,7 +220,7 @@ def run_b200(args):
 
     c = workload(args)
     L, N, R, mcs = c["L"], c["N"], c["R"], c["mcs_per_step"]
-    engine = {"auto": 0, "simple": 1, "warp": 2, "onchip": 3, "block": 4}[args.engine]
+    engine = {"auto": 0, "simple": 1, "warp": 2, "onchip": 3, "thread": 4}[args.engine]
     stream = torch.cuda.Stream()
     heights = torch.empty((R, L, L), dtype=torch.int32, device="cuda")      # device memory only: plumbing
     g = pkg.Rsos(L, N, R, c["seed"], tile=c["tile"], subsweeps=c["subsweeps"], first_real=rank * R, engine=engine,

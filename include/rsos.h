@@ -48,15 +48,22 @@ enum {
 
 /* Update engines.  All of them produce bit-identical heights (tests/test_gpu_parity.py).       */
 enum {
-    RSOS_ENGINE_AUTO   = 0,  /* ONCHIP when the mode is RS and the lattice fits in shared memory, */
-                             /* else WARP in DT mode, else SIMPLE                                 */
+    RSOS_ENGINE_AUTO   = 0,  /* RS mode: ONCHIP when the lattice fits in shared memory, else      */
+                             /* SIMPLE.  DT mode: THREAD when it applies and one colour pass has  */
+                             /* at least RSOS_THREAD_MIN_TILES active tiles, else WARP, else      */
+                             /* SIMPLE                                                            */
     RSOS_ENGINE_SIMPLE = 1,  /* one thread per active tile, heights in global memory (slow;       */
                              /* the literal loop nest of D:2, kept as an on-device cross-check)   */
     RSOS_ENGINE_WARP   = 2,  /* DT mode: one warp per active tile, (S+2)^2 window staged in       */
-                             /* shared memory, 32 attempts in flight with exact conflict votes    */
-    RSOS_ENGINE_ONCHIP = 3   /* RS mode (2S > L): one warp per realization, the whole lattice     */
+                             /* shared memory, 32 attempts in flight with exact conflict votes;   */
+                             /* needs tile <= 128 and N <= 31                                     */
+    RSOS_ENGINE_ONCHIP = 3,  /* RS mode (2S > L): one warp per realization, the whole lattice     */
                              /* stays in shared memory for all MCS of one rsos_advance call       */
+    RSOS_ENGINE_THREAD = 4   /* DT mode: one thread per active tile, the tile window held in      */
+                             /* bank-interleaved shared memory at 2 (N = 1) or 4 (N <= 7) bits    */
+                             /* per site; needs tile <= 64 and N <= 7                             */
 };
+#define RSOS_THREAD_MIN_TILES 4096u
 
 /* Options; all fields optional, zero = default.  Passed by pointer, copied by rsos_init.       */
 typedef struct rsos_opts {

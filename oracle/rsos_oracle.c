@@ -191,12 +191,11 @@ static int attempt_checked(rsos_oracle *c, int32_t *h, uint32_t x, uint32_t y)
 /* ------------------------------------------------------------------------------------------
  * All A attempts of one tile, in order a = 0 .. A-1.  S8c.1 step 6:
  *   slot width w = 16 if 2*lg(Se) <= 16 else 32; ns = 128/w slots per Philox call;
- *   lane = a & 31, batch = a >> 5, q = 32*(batch / ns) + lane, j = batch % ns;
+ *   q = a / ns (call index), j = a % ns (slot within the call): consecutive attempts consume
+ *   the slots of one call in order, then the next call (DESIGN.md section 2 step 6, reading Q16);
  *   o = Philox(counter = (q, tile id, u, r), key = seed);
  *   v = 16-bit slot j of o (low half first) or o[j];  dx = v & (Se-1), dy = (v >> lg Se) & (Se-1);
  *   site x = (ox + I*S + dx) & (L-1), y = (oy + J*S + dy) & (L-1).
- * The loop nest below (call block cb, slot j, lane) enumerates a = ((cb*ns + j)*32 + lane) in
- * increasing order, i.e. exactly a = 0 .. A-1, and evaluates each Philox call once.
  * General-L draw (L not a power of two; RS only; used by the 3x3 pin): w = 32 and
  *   site = ((uint64)v * L*L) >> 32, x = site % L, y = site / L.
  * Returns the number of accepted deposits.
@@ -210,26 +209,22 @@ static int64_t run_tile(rsos_oracle *c, int32_t *h, uint32_t rg, uint32_t u, uin
     const uint32_t ns = 128 / w;
     int64_t acc = 0;
     uint64_t a = 0;
-    for (uint32_t cb = 0; a < A; ++cb) {
-        uint32_t o[32][4];
-        for (uint32_t lane = 0; lane < 32; ++lane) {
-            uint32_t ctr[4] = { 32 * cb + lane, tile_id, u, rg };
-            rsos_oracle_philox(ctr, key, o[lane]);
-        }
-        for (uint32_t j = 0; j < ns && a < A; ++j)
-            for (uint32_t lane = 0; lane < 32 && a < A; ++lane, ++a) {
-                uint32_t v = (w == 16) ? (o[lane][j >> 1] >> (16 * (j & 1))) & 0xffffu : o[lane][j];
-                uint32_t x, y;
-                if (c->pow2) {
-                    uint32_t dx = v & (Se - 1), dy = (v >> lgSe) & (Se - 1);
-                    x = (x0 + dx) & (L - 1);
-                    y = (y0 + dy) & (L - 1);
-                } else {
-                    uint32_t site = (uint32_t)(((uint64_t)v * ((uint64_t)L * L)) >> 32);
-                    x = site % L; y = site / L;
-                }
-                acc += attempt_checked(c, h, x, y);
+    for (uint64_t q = 0; a < A; ++q) {
+        uint32_t ctr[4] = { (uint32_t)q, tile_id, u, rg }, o[4];
+        rsos_oracle_philox(ctr, key, o);
+        for (uint32_t j = 0; j < ns && a < A; ++j, ++a) {
+            uint32_t v = (w == 16) ? (o[j >> 1] >> (16 * (j & 1))) & 0xffffu : o[j];
+            uint32_t x, y;
+            if (c->pow2) {
+                uint32_t dx = v & (Se - 1), dy = (v >> lgSe) & (Se - 1);
+                x = (x0 + dx) & (L - 1);
+                y = (y0 + dy) & (L - 1);
+            } else {
+                uint32_t site = (uint32_t)(((uint64_t)v * ((uint64_t)L * L)) >> 32);
+                x = site % L; y = site / L;
             }
+            acc += attempt_checked(c, h, x, y);
+        }
     }
     return acc;
 }

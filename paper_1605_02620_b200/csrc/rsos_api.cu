@@ -95,7 +95,7 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
     if (N < 1 || N > 127) return fail(RSOS_EINVAL, "N = %u must be in [1, 127]", N);
     if (R < 1) return fail(RSOS_EINVAL, "R must be >= 1");
     if (opt.reserved) return fail(RSOS_EINVAL, "opts.reserved must be 0");
-    if (opt.engine > RSOS_ENGINE_ONCHIP) return fail(RSOS_EINVAL, "unknown engine %u", opt.engine);
+    if (opt.engine > RSOS_ENGINE_THREAD) return fail(RSOS_EINVAL, "unknown engine %u", opt.engine);
     uint32_t S = opt.tile ? opt.tile : 64, K = opt.subsweeps ? opt.subsweeps : 1;
     if (!is_pow2(S) || S < 8) return fail(RSOS_EINVAL, "tile = %u must be a power of two >= 8", S);
     if (!is_pow2(K)) return fail(RSOS_EINVAL, "subsweeps = %u must be a power of two", K);
@@ -112,11 +112,18 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
     // engine selection (include/rsos.h)
     uint32_t engine = opt.engine;
     const bool warp_ok = mode_dt && S <= 128 && N <= 31;
+    const bool thread_ok = mode_dt && S <= 64 && N <= 7;
     const bool onchip_ok = !mode_dt && L <= 128 && N <= 31;
-    if (engine == RSOS_ENGINE_AUTO) engine = mode_dt ? (warp_ok ? RSOS_ENGINE_WARP : RSOS_ENGINE_SIMPLE)
-                                                     : (onchip_ok ? RSOS_ENGINE_ONCHIP : RSOS_ENGINE_SIMPLE);
+    const uint64_t pass_tiles = mode_dt ? (uint64_t)R * (L / S / 2) * (L / S / 2) : 0;
+    if (engine == RSOS_ENGINE_AUTO) {
+        if (!mode_dt) engine = onchip_ok ? RSOS_ENGINE_ONCHIP : RSOS_ENGINE_SIMPLE;
+        else if (thread_ok && pass_tiles >= RSOS_THREAD_MIN_TILES) engine = RSOS_ENGINE_THREAD;
+        else engine = warp_ok ? RSOS_ENGINE_WARP : thread_ok ? RSOS_ENGINE_THREAD : RSOS_ENGINE_SIMPLE;
+    }
     if (engine == RSOS_ENGINE_WARP && !warp_ok)
         return fail(RSOS_EUNSUP, "engine WARP needs DT mode (2*tile <= L), tile <= 128 and N <= 31");
+    if (engine == RSOS_ENGINE_THREAD && !thread_ok)
+        return fail(RSOS_EUNSUP, "engine THREAD needs DT mode (2*tile <= L), tile <= 64 and N <= 7");
     if (engine == RSOS_ENGINE_ONCHIP && !onchip_ok)
         return fail(RSOS_EUNSUP, "engine ONCHIP needs RS mode (2*tile > L), L <= 128 and N <= 31");
 
@@ -166,7 +173,8 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
     INIT_TRY(configure_engine(p, engine, mode_dt), RSOS_ECUDA);
     INIT_TRY(cudaEventCreate(&c->ev0), RSOS_ECUDA);
     INIT_TRY(cudaEventCreate(&c->ev1), RSOS_ECUDA);
-    c->smem_bytes = engine == RSOS_ENGINE_WARP ? warp_dt_smem(p.lgS) : engine == RSOS_ENGINE_ONCHIP ? warp_rs_smem(p.lgL) : 0;
+    c->smem_bytes = engine == RSOS_ENGINE_WARP ? warp_dt_smem(p.lgS) : engine == RSOS_ENGINE_ONCHIP ? warp_rs_smem(p.lgL)
+                    : engine == RSOS_ENGINE_THREAD ? thread_dt_smem(p) : 0;
 #undef INIT_TRY
     *out = c;
     return RSOS_OK;

@@ -12,7 +12,7 @@ struct Params;
 constexpr int WARP_DT_WARPS = 8;     // warps (= tiles) per block of the DT warp engine
 constexpr int WARP_RS_WARPS = 4;     // warps (= realizations) per block of the on-chip RS engine
 
-enum : uint32_t { ENGINE_AUTO = 0, ENGINE_SIMPLE = 1, ENGINE_WARP = 2, ENGINE_ONCHIP = 3 };
+enum : uint32_t { ENGINE_AUTO = 0, ENGINE_SIMPLE = 1, ENGINE_WARP = 2, ENGINE_ONCHIP = 3, ENGINE_THREAD = 4 };
 
 // rsos_update.cu
 size_t warp_dt_smem(uint32_t lgS);
@@ -22,6 +22,13 @@ uint32_t engine_blocks(const Params &p, uint32_t engine, bool mode_dt);
 cudaError_t launch_dt_pass(const Params &p, uint32_t engine, uint32_t u, uint32_t colour, cudaStream_t st);
 cudaError_t launch_rs_sweeps(const Params &p, uint32_t engine, uint32_t t0, uint32_t mcs, cudaStream_t st);
 cudaError_t launch_philox(const uint32_t *d_ctr, const uint32_t *d_key, uint32_t *d_out, uint32_t n, cudaStream_t st);
+
+// rsos_thread.cu (lane-per-tile DT engine)
+bool thread_dt_supported(const Params &p);
+size_t thread_dt_smem(const Params &p);
+cudaError_t thread_dt_configure(const Params &p);
+uint32_t thread_dt_blocks(const Params &p);
+cudaError_t thread_dt_launch(const Params &p, uint32_t u, uint32_t colour, cudaStream_t st);
 
 // rsos_reduce.cu
 // out: per realization 4 x uint64: S1 (as int64 bits), S2, max |h| (max over threads), unused

@@ -32,10 +32,8 @@ __device__ __forceinline__ uint32_t simple_run_tile(const Params &p, int32_t *h,
     uint4 o = make_uint4(0, 0, 0, 0);
     uint32_t have_q = 0xFFFFFFFFu;
     for (uint64_t a = 0; a < A; ++a) {
-        const uint32_t lane = (uint32_t)a & 31u;
-        const uint32_t batch = (uint32_t)(a >> 5);
-        const uint32_t q = 32u * (batch >> lg_ns) + lane;
-        const uint32_t j = batch & ((1u << lg_ns) - 1u);
+        const uint32_t q = (uint32_t)(a >> lg_ns);                  // D:2 step 6: call a / ns, slot a % ns
+        const uint32_t j = (uint32_t)a & ((1u << lg_ns) - 1u);
         if (q != have_q) { o = philox4x32_10(q, tile_id, u, rg, p.k0, p.k1); have_q = q; }
         uint32_t v;
         if (w16) {
@@ -138,23 +136,28 @@ __device__ __forceinline__ uint32_t warp_run_attempts(uint32_t *sm, uint32_t A, 
     const uint32_t FULL = 0xFFFFFFFFu;
     const uint32_t TAG = lane_tag(lane);
     const uint32_t nbatch = (A + 31u) >> 5;
-    const uint32_t ncalls = (nbatch + 7u) >> 3;
     uint32_t my_acc = 0;
     uint32_t a0 = 0;
-    uint4 cur, nxt = philox4x32_10(lane, tile_id, u, rg, k0, k1);
-    for (uint32_t call = 0; call < ncalls; ++call) {
-        cur = nxt;
-        if (call + 1 < ncalls) nxt = philox4x32_10(32u * (call + 1) + lane, tile_id, u, rg, k0, k1);
-        for (uint32_t j0 = 0; j0 < 8; ++j0) {
-            const uint32_t batch = call * 8 + j0;
-            if (batch >= nbatch) break;
-            // 16-bit slots j0 (this batch) and j0 + 1 (the next batch: lanes that are already past
-            // the batch boundary); both are warp-uniform choices of register, hoisted per batch.
-            const uint32_t wA = (j0 & 4) ? ((j0 & 2) ? cur.w : cur.z) : ((j0 & 2) ? cur.y : cur.x);
-            const uint32_t vA = (wA >> (16u * (j0 & 1u))) & 0xFFFFu;
-            const uint32_t j1 = j0 + 1;
-            const uint32_t wB = (j1 & 8) ? nxt.x : (j1 & 4) ? ((j1 & 2) ? cur.w : cur.z) : ((j1 & 2) ? cur.y : cur.x);
-            const uint32_t vB = (wB >> (16u * (j1 & 1u))) & 0xFFFFu;
+    // D:2 step 6: attempt a takes the 16-bit slot a & 7 of Philox call a >> 3.  Lane l computes the
+    // calls 32 g + l of group g (256 attempts); attempt 32 b + l of batch b = 8 g + bb then reads
+    // slot l & 7 of the call held by lane 4 bb + (l >> 3) through shuffles.
+    const uint32_t sub = lane >> 3, wsel = (lane >> 1) & 3u, hsh = 16u * (lane & 1u);
+    auto slot = [&](const uint4 &c, uint32_t bb) -> uint32_t {
+        const uint32_t src = 4u * bb + sub;
+        const uint32_t x = __shfl_sync(FULL, c.x, src), y = __shfl_sync(FULL, c.y, src);
+        const uint32_t z = __shfl_sync(FULL, c.z, src), w = __shfl_sync(FULL, c.w, src);
+        const uint32_t word = (wsel & 2u) ? ((wsel & 1u) ? w : z) : ((wsel & 1u) ? y : x);
+        return (word >> hsh) & 0xFFFFu;
+    };
+    uint4 cur = philox4x32_10(lane, tile_id, u, rg, k0, k1), nxt = cur;
+    uint32_t vA = slot(cur, 0u), vB = 0u;
+    {
+        for (uint32_t batch = 0; batch < nbatch; ++batch) {
+            const uint32_t bb = batch & 7u;
+            if (bb == 0u && batch + 8u < nbatch)
+                nxt = philox4x32_10(32u * ((batch >> 3) + 1u) + lane, tile_id, u, rg, k0, k1);
+            // vA: slots of this batch; vB: slots of the next one (lanes already past the boundary)
+            if (batch + 1u < nbatch) vB = (bb < 7u) ? slot(cur, bb + 1u) : slot(nxt, 0u);
             const uint32_t batch_end = min((batch + 1u) << 5, A);
             while (a0 < batch_end) {
                 const uint32_t s = a0 & 31u;
@@ -212,6 +215,8 @@ __device__ __forceinline__ uint32_t warp_run_attempts(uint32_t *sm, uint32_t A, 
                 }
                 a0 += f;
             }
+            vA = vB;
+            if (bb == 7u) cur = nxt;
         }
     }
     return my_acc;
@@ -469,6 +474,7 @@ static cudaError_t dispatch_warp_rs(const Params &p, uint32_t t0, uint32_t mcs, 
 
 cudaError_t configure_engine(const Params &p, uint32_t engine, bool mode_dt)
 {
+    if (engine == ENGINE_THREAD && mode_dt) return thread_dt_configure(p);
     if (engine == ENGINE_WARP && mode_dt) return dispatch_warp_dt(p, 0, 0, 0, nullptr, true);
     if (engine == ENGINE_ONCHIP && !mode_dt) return dispatch_warp_rs(p, 0, 0, 0, nullptr, true);
     return cudaSuccess;
@@ -478,6 +484,7 @@ uint32_t engine_blocks(const Params &p, uint32_t engine, bool mode_dt)
 {
     const uint32_t T = p.L >> p.lgS, half = T >> 1;
     const uint64_t tiles = mode_dt ? (uint64_t)p.R * half * half : p.R;
+    if (engine == ENGINE_THREAD) return thread_dt_blocks(p);
     if (engine == ENGINE_WARP) return (uint32_t)((tiles + WARP_DT_WARPS - 1) / WARP_DT_WARPS);
     if (engine == ENGINE_ONCHIP) return (uint32_t)((tiles + WARP_RS_WARPS - 1) / WARP_RS_WARPS);
     return (uint32_t)((tiles + (mode_dt ? 127 : 31)) / (mode_dt ? 128 : 32));
@@ -486,6 +493,7 @@ uint32_t engine_blocks(const Params &p, uint32_t engine, bool mode_dt)
 // One colour pass of sub-sweep u (DT mode).
 cudaError_t launch_dt_pass(const Params &p, uint32_t engine, uint32_t u, uint32_t colour, cudaStream_t st)
 {
+    if (engine == ENGINE_THREAD) return thread_dt_launch(p, u, colour, st);
     const uint32_t blocks = engine_blocks(p, engine, true);
     if (engine == ENGINE_WARP) return dispatch_warp_dt(p, u, colour, blocks, st, false);
     simple_dt_kernel<<<blocks, 128, 0, st>>>(p, u, colour);

@@ -89,6 +89,40 @@ def test_dt_warp_engine_equals_oracle(rsos, oracle_mod, L, N, R, S, K, mcs, seed
     g.close()
 
 
+@pytest.mark.parametrize("L,N,R,S,K,mcs,seed", [
+    (128, 1, 3, 64, 1, 6, 1),        # one tile per colour per realization: 3 live lanes, 29 idle ones
+    (256, 1, 5, 64, 1, 5, 2),        # lanes of one warp span realizations with different origins
+    (512, 1, 3, 64, 1, 4, 12),       # 48 tiles per pass: two warps, ragged tail
+    (256, 2, 2, 64, 4, 4, 3),        # 4-bit sites (N = 2), K = 4 sub-sweeps
+    (256, 4, 1, 64, 1, 4, 4),        # config C3 slopes
+    (512, 7, 1, 64, 2, 3, 5),        # largest N of the 4-bit format
+    (128, 1, 2, 32, 4, 5, 6),        # S = 32
+    (64, 2, 3, 16, 1, 5, 7),         # S = 16
+    (64, 1, 2, 8, 2, 5, 8),          # S = 8, A = 32 attempts per tile
+    (128, 1, 1, 64, 128, 2, 11),     # A = 32
+])
+def test_dt_thread_engine_equals_oracle(rsos, oracle_mod, L, N, R, S, K, mcs, seed):
+    """The lane-per-tile engine (2- or 4-bit sites, bank-interleaved shared memory)."""
+    g = rsos.Rsos(L, N, R, seed, tile=S, subsweeps=K, engine=rsos.ENGINE_THREAD)
+    o = oracle_mod.Oracle(L, N, R, seed, tile=S, subsweeps=K)
+    assert g.info()["mode"] == "DT" and g.info()["engine"] == "thread"
+    for step in range(mcs):
+        g.advance(1)
+        o.advance(1)
+        compare(g, o, "DT thread L=%d N=%d S=%d K=%d t=%d" % (L, N, S, K, step + 1))
+    g.close()
+
+
+def test_dt_thread_engine_many_tiles_equals_warp_and_oracle_sample(rsos, oracle_mod):
+    """L = 2048, R = 2: 512 tiles per pass (16 warps).  Full heights against the oracle."""
+    g = rsos.Rsos(2048, 1, 2, 13, engine=rsos.ENGINE_THREAD)
+    o = oracle_mod.Oracle(2048, 1, 2, 13)
+    g.advance(2)
+    o.advance(2)
+    compare(g, o, "DT thread L=2048")
+    g.close()
+
+
 @pytest.mark.parametrize("L,N,R,S,K,mcs", [(128, 1, 2, 64, 1, 3), (128, 2, 2, 16, 4, 3), (1024, 1, 1, 512, 1, 1),
                                            (128, 40, 1, 64, 1, 2)])
 def test_dt_simple_engine_equals_oracle(rsos, oracle_mod, L, N, R, S, K, mcs):
