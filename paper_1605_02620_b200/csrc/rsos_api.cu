@@ -27,6 +27,8 @@ struct rsos_ctx {
     unsigned long long *h_red;        // pinned mirror
     long long *d_base;                // R int64 (moments)
     int sm_count;
+    uint32_t blocks;                  // update-kernel blocks per launch
+    uint32_t aux;                     // engine-specific launch argument (THREAD: prefetch stride)
     size_t smem_bytes;
     // optional timing of rsos_advance
     bool timing;
@@ -171,6 +173,8 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
     INIT_TRY(cudaMemsetAsync(p.err, 0, sizeof(uint32_t), c->stream), RSOS_ECUDA);
     INIT_TRY(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev), RSOS_ECUDA);
     INIT_TRY(configure_engine(p, engine, mode_dt), RSOS_ECUDA);
+    if (engine == RSOS_ENGINE_THREAD) INIT_TRY(thread_dt_grid(p, c->sm_count, &c->blocks, &c->aux), RSOS_ECUDA);
+    else c->blocks = engine_blocks(p, engine, mode_dt);
     INIT_TRY(cudaEventCreate(&c->ev0), RSOS_ECUDA);
     INIT_TRY(cudaEventCreate(&c->ev1), RSOS_ECUDA);
     c->smem_bytes = engine == RSOS_ENGINE_WARP ? warp_dt_smem(p.lgS) : engine == RSOS_ENGINE_ONCHIP ? warp_rs_smem(p.lgL)
@@ -222,12 +226,12 @@ extern "C" int rsos_advance(rsos_ctx *c, uint64_t mcs)
             for (uint32_t k = 0; k < p.K; ++k) {
                 const uint32_t u = (uint32_t)((c->t + m) * p.K + k);
                 for (uint32_t colour = 0; colour < 4; ++colour) {
-                    CUDA_TRY(launch_dt_pass(p, c->engine, u, colour, c->stream));
+                    CUDA_TRY(launch_dt_pass(p, c->engine, u, colour, c->blocks, c->aux, c->stream));
                     ++c->launches;
                 }
             }
     } else {
-        CUDA_TRY(launch_rs_sweeps(p, c->engine, (uint32_t)c->t, (uint32_t)mcs, c->stream));
+        CUDA_TRY(launch_rs_sweeps(p, c->engine, (uint32_t)c->t, (uint32_t)mcs, c->blocks, c->stream));
         ++c->launches;
     }
     if (c->timing) {
@@ -374,7 +378,7 @@ extern "C" int rsos_info(rsos_ctx *c, uint64_t *out)
     out[4] = c->launches;
     out[5] = (uint64_t)c->sm_count;
     out[6] = c->smem_bytes;
-    out[7] = engine_blocks(c->p, c->engine, c->mode_dt);
+    out[7] = c->blocks;
     return RSOS_OK;
 }
 

@@ -68,18 +68,21 @@ __device__ __forceinline__ uint32_t thread_attempt(uint32_t base, uint32_t dx, u
     asm volatile("ld.shared.u32 %0, [%1+128];" : "=r"(w1) : "r"(a0));
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(wu) : "r"(ac - G::ROWB));
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(wd) : "r"(ac + G::ROWB));
-    const uint32_t t3 = __funnelshift_r(w0, w1, bl & 31u);        // fields: L, C, R
     const uint32_t sc = bc & 31u;
-    const uint32_t hc = (t3 >> FB) & M;
-    const uint32_t t = (hc - N) & M;                              // a neighbour at h - N blocks (D:3 (i))
-    const bool blocked = ((t3 ^ t) & M) == 0u || (((t3 >> (2 * FB)) ^ t) & M) == 0u ||
-                         (((wu >> sc) ^ t) & M) == 0u || (((wd >> sc) ^ t) & M) == 0u;
-    if (!blocked) {
-        const uint32_t own = (bc >> 5) == (bl >> 5) ? w0 : w1;
-        const uint32_t nw = own ^ (((hc ^ (hc + 1u)) & M) << sc);
-        asm volatile("st.shared.u32 [%0], %1;" :: "r"(ac), "r"(nw) : "memory");
-    }
-    return blocked ? 0u : 1u;
+    const uint32_t t3 = __funnelshift_r(w0, w1, bl & 31u);        // fields: L, C, R (garbage above)
+    const uint32_t c = t3 >> FB;                                  // C in the low FB bits
+    // Under Eq. (6) the deposit is rejected iff some neighbour sits at h - N, i.e. (C - nb) mod 2^FB == N
+    // (D:3 (i)).  Branch-free: four independent subtract / test pairs.
+    const uint32_t okL = ((c - t3) ^ N) & M;
+    const uint32_t okR = ((c - (t3 >> (2 * FB))) ^ N) & M;
+    const uint32_t okU = ((c - (wu >> sc)) ^ N) & M;
+    const uint32_t okD = ((c - (wd >> sc)) ^ N) & M;
+    const bool ok = (okL != 0u) & (okR != 0u) & (okU != 0u) & (okD != 0u);
+    const uint32_t own = (bc >> 5) == (bl >> 5) ? w0 : w1;
+    const uint32_t nw = own ^ (((c ^ (c + 1u)) & M) << sc);       // field + 1 mod 2^FB
+    asm volatile("{ .reg .pred p; setp.ne.u32 p, %2, 0; @p st.shared.u32 [%0], %1; }"
+                 :: "r"(ac), "r"(nw), "r"((uint32_t)ok) : "memory");
+    return ok ? 1u : 0u;
 }
 
 template <int LGS, int FB>
@@ -192,30 +195,37 @@ __global__ void __launch_bounds__(32) thread_dt_kernel(Params p, uint32_t u, uin
 // Host-side launchers
 // =============================================================================================
 template <int LGS, int FB>
-static cudaError_t thread_dt_t(const Params &p, uint32_t u, uint32_t colour, uint32_t blocks, cudaStream_t st, int what,
-                               size_t *smem_out)
+static cudaError_t thread_dt_t(const Params &p, uint32_t u, uint32_t colour, uint32_t blocks, uint32_t pf_stride,
+                               cudaStream_t st, int what, size_t *out)
 {
     const size_t sm = (size_t)32 * TGeom<LGS, FB>::WORDS * 4;
-    if (what == 0) { *smem_out = sm; return cudaSuccess; }
+    if (what == 0) { *out = sm; return cudaSuccess; }
     if (what == 1)
         return cudaFuncSetAttribute(thread_dt_kernel<LGS, FB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    if (what == 3) {                                      // resident blocks per SM
+        int nb = 0;
+        const cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, thread_dt_kernel<LGS, FB>, 32, sm);
+        *out = (size_t)nb;
+        return e;
+    }
+    (void)pf_stride;
     thread_dt_kernel<LGS, FB><<<blocks, 32, sm, st>>>(p, u, colour);
     return cudaGetLastError();
 }
 
-static cudaError_t thread_dispatch(const Params &p, uint32_t u, uint32_t colour, uint32_t blocks, cudaStream_t st,
-                                   int what, size_t *smem_out)
+static cudaError_t thread_dispatch(const Params &p, uint32_t u, uint32_t colour, uint32_t blocks, uint32_t pf_stride,
+                                   cudaStream_t st, int what, size_t *out)
 {
     const bool two = p.N <= 1;
     switch (p.lgS) {
-        case 3: return two ? thread_dt_t<3, 2>(p, u, colour, blocks, st, what, smem_out)
-                           : thread_dt_t<3, 4>(p, u, colour, blocks, st, what, smem_out);
-        case 4: return two ? thread_dt_t<4, 2>(p, u, colour, blocks, st, what, smem_out)
-                           : thread_dt_t<4, 4>(p, u, colour, blocks, st, what, smem_out);
-        case 5: return two ? thread_dt_t<5, 2>(p, u, colour, blocks, st, what, smem_out)
-                           : thread_dt_t<5, 4>(p, u, colour, blocks, st, what, smem_out);
-        case 6: return two ? thread_dt_t<6, 2>(p, u, colour, blocks, st, what, smem_out)
-                           : thread_dt_t<6, 4>(p, u, colour, blocks, st, what, smem_out);
+        case 3: return two ? thread_dt_t<3, 2>(p, u, colour, blocks, pf_stride, st, what, out)
+                           : thread_dt_t<3, 4>(p, u, colour, blocks, pf_stride, st, what, out);
+        case 4: return two ? thread_dt_t<4, 2>(p, u, colour, blocks, pf_stride, st, what, out)
+                           : thread_dt_t<4, 4>(p, u, colour, blocks, pf_stride, st, what, out);
+        case 5: return two ? thread_dt_t<5, 2>(p, u, colour, blocks, pf_stride, st, what, out)
+                           : thread_dt_t<5, 4>(p, u, colour, blocks, pf_stride, st, what, out);
+        case 6: return two ? thread_dt_t<6, 2>(p, u, colour, blocks, pf_stride, st, what, out)
+                           : thread_dt_t<6, 4>(p, u, colour, blocks, pf_stride, st, what, out);
         default: return cudaErrorInvalidValue;
     }
 }
@@ -225,22 +235,34 @@ bool thread_dt_supported(const Params &p) { return p.lgS >= 3 && p.lgS <= 6 && p
 size_t thread_dt_smem(const Params &p)
 {
     size_t sm = 0;
-    thread_dispatch(p, 0, 0, 0, nullptr, 0, &sm);
+    thread_dispatch(p, 0, 0, 0, 0, nullptr, 0, &sm);
     return sm;
 }
 
-cudaError_t thread_dt_configure(const Params &p) { return thread_dispatch(p, 0, 0, 0, nullptr, 1, nullptr); }
+cudaError_t thread_dt_configure(const Params &p) { return thread_dispatch(p, 0, 0, 0, 0, nullptr, 1, nullptr); }
 
-uint32_t thread_dt_blocks(const Params &p)
+// One block per tile set (the hardware block scheduler balances sets of unequal duration better
+// than a static stride).  pf_stride = resident blocks of the device: when block b is running, block
+// b + pf_stride is (about) the one that will take over its slot, so that is the set b prefetches.
+cudaError_t thread_dt_grid(const Params &p, int sm_count, uint32_t *blocks, uint32_t *pf_stride)
 {
     const uint32_t T = p.L >> p.lgS, half = T >> 1;
     const uint64_t tiles = (uint64_t)p.R * half * half;
-    return (uint32_t)((tiles + 31) / 32);
+    const uint64_t nsets = (tiles + 31) / 32;
+    size_t per_sm = 0;
+    const cudaError_t e = thread_dispatch(p, 0, 0, 0, 0, nullptr, 3, &per_sm);
+    if (e != cudaSuccess) return e;
+    if (per_sm == 0) return cudaErrorLaunchOutOfResources;
+    const uint64_t slots = (uint64_t)sm_count * per_sm;
+    *blocks = (uint32_t)nsets;
+    *pf_stride = nsets > slots ? (uint32_t)slots : 0u;
+    return cudaSuccess;
 }
 
-cudaError_t thread_dt_launch(const Params &p, uint32_t u, uint32_t colour, cudaStream_t st)
+cudaError_t thread_dt_launch(const Params &p, uint32_t u, uint32_t colour, uint32_t blocks, uint32_t pf_stride,
+                             cudaStream_t st)
 {
-    return thread_dispatch(p, u, colour, thread_dt_blocks(p), st, 2, nullptr);
+    return thread_dispatch(p, u, colour, blocks, pf_stride, st, 2, nullptr);
 }
 
 }  // namespace rsos
