@@ -28,7 +28,12 @@ struct rsos_ctx {
     long long *d_base;                // R int64 (moments)
     int sm_count;
     uint32_t blocks;                  // update-kernel blocks per launch
-    uint32_t aux;                     // engine-specific launch argument (THREAD: prefetch stride)
+    // THREAD engine: the working state is the packed lattice p.pk; the int32 heights p.h are rebuilt on demand
+    bool h_valid, pk_valid;           // which of the two copies is current (both after init)
+    long long *d_s1off;               // R int64: sum h = s1off + accepted while pk is the current copy
+    int32_t *d_V;                     // R * L int32 scratch (column chain)
+    unsigned long long *d_srel;       // R uint64 scratch
+    int32_t *d_h00;                   // R int32 scratch
     size_t smem_bytes;
     // optional timing of rsos_advance
     bool timing;
@@ -81,6 +86,11 @@ static void destroy(rsos_ctx *c)
     if (c->d_red) cudaFree(c->d_red);
     if (c->h_red) cudaFreeHost(c->h_red);
     if (c->d_base) cudaFree(c->d_base);
+    if (c->p.pk) cudaFree(c->p.pk);
+    if (c->d_s1off) cudaFree(c->d_s1off);
+    if (c->d_V) cudaFree(c->d_V);
+    if (c->d_srel) cudaFree(c->d_srel);
+    if (c->d_h00) cudaFree(c->d_h00);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
     delete c;
@@ -168,13 +178,24 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
     INIT_TRY(cudaMalloc(&c->d_red, (size_t)R * 8 * sizeof(unsigned long long)), RSOS_ECUDA);
     INIT_TRY(cudaMallocHost(&c->h_red, (size_t)R * 8 * sizeof(unsigned long long)), RSOS_ECUDA);
     INIT_TRY(cudaMalloc(&c->d_base, (size_t)R * sizeof(long long)), RSOS_ECUDA);
+    c->h_valid = c->pk_valid = true;
+    if (engine == RSOS_ENGINE_THREAD) {
+        p.FB = thread_dt_field_bits(N, S);
+        const size_t pk_bytes = bytes / 32 * p.FB;                       // FB bits per site
+        INIT_TRY(cudaMalloc(&p.pk, pk_bytes), RSOS_ECUDA);
+        INIT_TRY(cudaMalloc(&c->d_s1off, (size_t)R * sizeof(long long)), RSOS_ECUDA);
+        INIT_TRY(cudaMalloc(&c->d_V, (size_t)R * L * sizeof(int32_t)), RSOS_ECUDA);
+        INIT_TRY(cudaMalloc(&c->d_srel, (size_t)R * sizeof(unsigned long long)), RSOS_ECUDA);
+        INIT_TRY(cudaMalloc(&c->d_h00, (size_t)R * sizeof(int32_t)), RSOS_ECUDA);
+        INIT_TRY(cudaMemsetAsync(p.pk, 0, pk_bytes, c->stream), RSOS_ECUDA);                // flat start
+        INIT_TRY(cudaMemsetAsync(c->d_s1off, 0, (size_t)R * sizeof(long long), c->stream), RSOS_ECUDA);
+    }
     INIT_TRY(cudaMemsetAsync(p.h, 0, bytes, c->stream), RSOS_ECUDA);                 // flat start
     INIT_TRY(cudaMemsetAsync(p.accepted, 0, (size_t)R * sizeof(unsigned long long), c->stream), RSOS_ECUDA);
     INIT_TRY(cudaMemsetAsync(p.err, 0, sizeof(uint32_t), c->stream), RSOS_ECUDA);
     INIT_TRY(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev), RSOS_ECUDA);
     INIT_TRY(configure_engine(p, engine, mode_dt), RSOS_ECUDA);
-    if (engine == RSOS_ENGINE_THREAD) INIT_TRY(thread_dt_grid(p, c->sm_count, &c->blocks, &c->aux), RSOS_ECUDA);
-    else c->blocks = engine_blocks(p, engine, mode_dt);
+    c->blocks = engine_blocks(p, engine, mode_dt);
     INIT_TRY(cudaEventCreate(&c->ev0), RSOS_ECUDA);
     INIT_TRY(cudaEventCreate(&c->ev1), RSOS_ECUDA);
     c->smem_bytes = engine == RSOS_ENGINE_WARP ? warp_dt_smem(p.lgS) : engine == RSOS_ENGINE_ONCHIP ? warp_rs_smem(p.lgL)
@@ -205,6 +226,30 @@ static int flush_timing(rsos_ctx *c)
     return RSOS_OK;
 }
 
+// THREAD engine: make the int32 heights current (packed lattice -> p.h, rsos_pack.cu).
+static int ensure_heights(rsos_ctx *c)
+{
+    if (!c->p.pk || c->h_valid) return RSOS_OK;
+    uint32_t n = 0;
+    CUDA_TRY(launch_unpack(c->p, c->d_s1off, c->d_V, c->d_srel, c->d_h00, c->stream, &n));
+    c->launches += n;
+    c->h_valid = true;
+    return RSOS_OK;
+}
+
+// THREAD engine: make the packed lattice current (p.h -> packed, and s1off = sum h - accepted).
+static int ensure_packed(rsos_ctx *c)
+{
+    if (!c->p.pk || c->pk_valid) return RSOS_OK;
+    const Params &p = c->p;
+    CUDA_TRY(launch_sums(p.h, p.L, p.R, c->d_red, c->stream));
+    CUDA_TRY(launch_s1off(p, c->d_red, c->d_s1off, c->stream));
+    CUDA_TRY(launch_pack(p, c->stream));
+    c->launches += (p.R + 65534) / 65535 + 2;
+    c->pk_valid = true;
+    return RSOS_OK;
+}
+
 extern "C" int rsos_advance(rsos_ctx *c, uint64_t mcs)
 {
     if (!c) return fail(RSOS_EINVAL, "ctx is NULL");
@@ -221,12 +266,17 @@ extern "C" int rsos_advance(rsos_ctx *c, uint64_t mcs)
         CUDA_TRY(cudaEventRecord(c->ev0, c->stream));
         c->launches_at_ev0 = c->launches;
     }
+    if (c->p.pk) {
+        const int rc = ensure_packed(c);
+        if (rc) return rc;
+        c->h_valid = false;
+    }
     if (c->mode_dt) {
         for (uint64_t m = 0; m < mcs; ++m)
             for (uint32_t k = 0; k < p.K; ++k) {
                 const uint32_t u = (uint32_t)((c->t + m) * p.K + k);
                 for (uint32_t colour = 0; colour < 4; ++colour) {
-                    CUDA_TRY(launch_dt_pass(p, c->engine, u, colour, c->blocks, c->aux, c->stream));
+                    CUDA_TRY(launch_dt_pass(p, c->engine, u, colour, c->blocks, c->stream));
                     ++c->launches;
                 }
             }
@@ -254,6 +304,10 @@ static int check_device_err(rsos_ctx *c)
 static int reduce_sums(rsos_ctx *c)
 {
     const Params &p = c->p;
+    {
+        const int rc0 = ensure_heights(c);
+        if (rc0) return rc0;
+    }
     CUDA_TRY(launch_sums(p.h, p.L, p.R, c->d_red, c->stream));
     c->launches += (p.R + 65534) / 65535;
     CUDA_TRY(cudaMemcpyAsync(c->h_red, c->d_red, (size_t)p.R * 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
@@ -338,6 +392,10 @@ extern "C" int rsos_get_heights(rsos_ctx *c, uint32_t r0, uint32_t nr, int32_t *
     if (nr && !host_out) return fail(RSOS_EINVAL, "host_out is NULL");
     DeviceGuard guard(c->device);
     if (!guard.ok) return fail(RSOS_ECUDA, "cannot select CUDA device %d", c->device);
+    {
+        const int rc0 = ensure_heights(c);
+        if (rc0) return rc0;
+    }
     const size_t per = (size_t)c->p.L * c->p.L;
     if (nr) CUDA_TRY(cudaMemcpyAsync(host_out, c->p.h + r0 * per, nr * per * sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));
     return check_device_err(c);
@@ -352,6 +410,11 @@ extern "C" int rsos_set_state(rsos_ctx *c, uint32_t r0, uint32_t nr, const int32
     if (t * c->p.K >= (1ull << 32)) return fail(RSOS_ERANGE, "t * K reaches 2^32");
     DeviceGuard guard(c->device);
     if (!guard.ok) return fail(RSOS_ECUDA, "cannot select CUDA device %d", c->device);
+    {
+        const int rc0 = ensure_heights(c);                 // realizations outside [r0, r0+nr) keep their state
+        if (rc0) return rc0;
+        c->pk_valid = false;
+    }
     const size_t per = (size_t)c->p.L * c->p.L;
     if (nr) CUDA_TRY(cudaMemcpyAsync(c->p.h + r0 * per, host_in, nr * per * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
     if (nr && accepted)
@@ -385,6 +448,12 @@ extern "C" int rsos_info(rsos_ctx *c, uint64_t *out)
 extern "C" int rsos_device_heights(rsos_ctx *c, int32_t **d)
 {
     if (!c || !d) return fail(RSOS_EINVAL, "NULL argument");
+    {
+        DeviceGuard guard(c->device);
+        if (!guard.ok) return fail(RSOS_ECUDA, "cannot select CUDA device %d", c->device);
+        const int rc0 = ensure_heights(c);
+        if (rc0) return rc0;
+    }
     *d = c->p.h;
     return RSOS_OK;
 }

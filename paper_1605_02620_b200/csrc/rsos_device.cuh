@@ -44,10 +44,12 @@ struct Params {
     uint32_t S, lgS, K;             // tile side, sub-sweeps per MCS (DT); S = L, K = 1 in RS mode
     uint32_t k0, k1;                // Philox key = (seed lo, seed hi)
     uint32_t *err;                  // device error word (bit flags), see ERR_*
+    uint32_t *pk;                   // THREAD engine: packed working lattice, FB bits per site (rsos_pack.cu)
+    uint32_t FB;                    // field bits of pk (2 or 4); 0 when there is no packed lattice
 };
 
 enum : uint32_t {
-    ERR_RECONSTRUCT = 1u,           // on-chip engine: height reconstruction did not divide exactly
+    ERR_RECONSTRUCT = 1u,           // height reconstruction from differences did not divide exactly
 };
 
 // D:2 step 4: origin of sub-sweep u for realization rg: Philox counter (0, 0xFFFFFFFF, u, rg).

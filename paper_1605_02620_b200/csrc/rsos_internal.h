@@ -19,18 +19,22 @@ size_t warp_dt_smem(uint32_t lgS);
 size_t warp_rs_smem(uint32_t lgL);
 cudaError_t configure_engine(const Params &p, uint32_t engine, bool mode_dt);
 uint32_t engine_blocks(const Params &p, uint32_t engine, bool mode_dt);
-cudaError_t launch_dt_pass(const Params &p, uint32_t engine, uint32_t u, uint32_t colour, uint32_t blocks, uint32_t aux,
-                           cudaStream_t st);
+cudaError_t launch_dt_pass(const Params &p, uint32_t engine, uint32_t u, uint32_t colour, uint32_t blocks, cudaStream_t st);
 cudaError_t launch_rs_sweeps(const Params &p, uint32_t engine, uint32_t t0, uint32_t mcs, uint32_t blocks, cudaStream_t st);
 cudaError_t launch_philox(const uint32_t *d_ctr, const uint32_t *d_key, uint32_t *d_out, uint32_t n, cudaStream_t st);
 
-// rsos_thread.cu (lane-per-tile DT engine)
-bool thread_dt_supported(const Params &p);
+// rsos_thread.cu (lane-per-tile DT engine on the packed lattice)
+uint32_t thread_dt_field_bits(uint32_t N, uint32_t S);
 size_t thread_dt_smem(const Params &p);
 cudaError_t thread_dt_configure(const Params &p);
-cudaError_t thread_dt_grid(const Params &p, int sm_count, uint32_t *blocks, uint32_t *pf_stride);
-cudaError_t thread_dt_launch(const Params &p, uint32_t u, uint32_t colour, uint32_t blocks, uint32_t pf_stride,
-                             cudaStream_t st);
+uint32_t thread_dt_blocks(const Params &p);
+cudaError_t thread_dt_launch(const Params &p, uint32_t u, uint32_t colour, uint32_t blocks, cudaStream_t st);
+
+// rsos_pack.cu (packed working lattice <-> int32 heights)
+cudaError_t launch_pack(const Params &p, cudaStream_t st);
+cudaError_t launch_s1off(const Params &p, const unsigned long long *d_red, long long *d_s1off, cudaStream_t st);
+cudaError_t launch_unpack(const Params &p, const long long *d_s1off, int32_t *d_V, unsigned long long *d_srel,
+                          int32_t *d_h00, cudaStream_t st, uint32_t *launches);
 
 // rsos_reduce.cu
 // out: per realization 4 x uint64: S1 (as int64 bits), S2, max |h| (max over threads), unused

@@ -484,16 +484,16 @@ uint32_t engine_blocks(const Params &p, uint32_t engine, bool mode_dt)
 {
     const uint32_t T = p.L >> p.lgS, half = T >> 1;
     const uint64_t tiles = mode_dt ? (uint64_t)p.R * half * half : p.R;
+    if (engine == ENGINE_THREAD) return thread_dt_blocks(p);
     if (engine == ENGINE_WARP) return (uint32_t)((tiles + WARP_DT_WARPS - 1) / WARP_DT_WARPS);
     if (engine == ENGINE_ONCHIP) return (uint32_t)((tiles + WARP_RS_WARPS - 1) / WARP_RS_WARPS);
     return (uint32_t)((tiles + (mode_dt ? 127 : 31)) / (mode_dt ? 128 : 32));
 }
 
 // One colour pass of sub-sweep u (DT mode).
-cudaError_t launch_dt_pass(const Params &p, uint32_t engine, uint32_t u, uint32_t colour, uint32_t blocks, uint32_t aux,
-                           cudaStream_t st)
+cudaError_t launch_dt_pass(const Params &p, uint32_t engine, uint32_t u, uint32_t colour, uint32_t blocks, cudaStream_t st)
 {
-    if (engine == ENGINE_THREAD) return thread_dt_launch(p, u, colour, blocks, aux, st);
+    if (engine == ENGINE_THREAD) return thread_dt_launch(p, u, colour, blocks, st);
     if (engine == ENGINE_WARP) return dispatch_warp_dt(p, u, colour, blocks, st, false);
     simple_dt_kernel<<<blocks, 128, 0, st>>>(p, u, colour);
     return cudaGetLastError();

@@ -113,14 +113,41 @@ def test_dt_thread_engine_equals_oracle(rsos, oracle_mod, L, N, R, S, K, mcs, se
     g.close()
 
 
-def test_dt_thread_engine_many_tiles_equals_warp_and_oracle_sample(rsos, oracle_mod):
-    """L = 2048, R = 2: 512 tiles per pass (16 warps).  Full heights against the oracle."""
-    g = rsos.Rsos(2048, 1, 2, 13, engine=rsos.ENGINE_THREAD)
-    o = oracle_mod.Oracle(2048, 1, 2, 13)
-    g.advance(2)
-    o.advance(2)
-    compare(g, o, "DT thread L=2048")
+@pytest.mark.parametrize("L,N,R,mcs", [(2048, 1, 2, 2),     # 512 tiles per pass; rows rebuilt by one warp each
+                                       (4096, 1, 1, 1),     # 256 packed words per row: rows rebuilt by a whole block
+                                       (2048, 3, 1, 1)])    # 4-bit sites, 256 words per row
+def test_dt_thread_engine_large_lattices(rsos, oracle_mod, L, N, R, mcs):
+    """Many tiles per pass and both row-team shapes of the packed -> int32 rebuild (rsos_pack.cu)."""
+    g = rsos.Rsos(L, N, R, 13, engine=rsos.ENGINE_THREAD)
+    o = oracle_mod.Oracle(L, N, R, 13)
+    g.advance(mcs)
+    o.advance(mcs)
+    compare(g, o, "DT thread L=%d N=%d" % (L, N))
     g.close()
+
+
+def test_dt_thread_engine_snapshot_restart(rsos, oracle_mod):
+    """Packed working lattice: heights read back mid-run, a snapshot written into SOME realizations
+    (rsos_set_state) and the run continued; every realization must still follow the oracle."""
+    L, N, R, seed = 256, 1, 4, 31
+    g = rsos.Rsos(L, N, R, seed, engine=rsos.ENGINE_THREAD)
+    o = oracle_mod.Oracle(L, N, R, seed)
+    g.advance(3)
+    o.advance(3)
+    compare(g, o, "before snapshot")
+    h = o.heights()
+    acc = o.sums()[2]
+    g2 = rsos.Rsos(L, N, R, seed, engine=rsos.ENGINE_THREAD)
+    g2.advance(1)                                           # some other state, to be overwritten
+    g2.set_state(h, 3, acc)
+    g.set_state(h[1:3], 3, acc[1:3], r0=1)                  # rewrite realizations 1, 2 with their own state
+    for x in (g, g2):
+        x.advance(2)
+    o.advance(2)
+    compare(g, o, "after partial set_state")
+    compare(g2, o, "restart from snapshot")
+    g.close()
+    g2.close()
 
 
 @pytest.mark.parametrize("L,N,R,S,K,mcs", [(128, 1, 2, 64, 1, 3), (128, 2, 2, 16, 4, 3), (1024, 1, 1, 512, 1, 1),
