@@ -49,6 +49,7 @@ def parse():
     ap.add_argument("--workload", default="C2", choices=sorted(workloads.CONFIGS))
     ap.add_argument("--mcs-per-step", type=int, default=0, help="MCS per step (0 = workload default)")
     ap.add_argument("--engine", default="auto", choices=["auto", "simple", "warp", "onchip", "thread"])
+    ap.add_argument("--lanes", type=int, default=0, help="THREAD engine lanes per tile (0 = auto)")
     ap.add_argument("--tile", type=int, default=0)
     ap.add_argument("--subsweeps", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -224,7 +225,7 @@ def run_b200(args):
     stream = torch.cuda.Stream()
     heights = torch.empty((R, L, L), dtype=torch.int32, device="cuda")      # device memory only: plumbing
     g = pkg.Rsos(L, N, R, c["seed"], tile=c["tile"], subsweeps=c["subsweeps"], first_real=rank * R, engine=engine,
-                 d_heights=heights.data_ptr(), stream=stream.cuda_stream)
+                 d_heights=heights.data_ptr(), stream=stream.cuda_stream, lanes=args.lanes)
     info = g.info()
     att_step = workloads.attempts(L, R, mcs)
 

@@ -77,7 +77,8 @@ typedef struct rsos_opts {
                           /* Its content on entry is ignored: rsos_init zeroes it (flat start).   */
     void    *stream;      /* cudaStream_t to enqueue on; NULL = the legacy default stream         */
     int32_t  device;      /* CUDA device ordinal + 1; 0 = the current device                      */
-    uint32_t reserved;    /* must be 0                                                            */
+    uint32_t lanes;       /* THREAD engine: lanes that share one tile, 1, 2 or 4; 0 = chosen from the     */
+                          /* number of tiles per colour pass (D:4).  Does not change the result.          */
 } rsos_opts;
 
 /*

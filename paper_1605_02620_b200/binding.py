@@ -25,7 +25,7 @@ SYMBOLS = ("rsos_init", "rsos_advance", "rsos_sums", "rsos_width", "rsos_moments
 class RsosOpts(C.Structure):
     _fields_ = [("tile", C.c_uint32), ("subsweeps", C.c_uint32), ("first_real", C.c_uint32),
                 ("engine", C.c_uint32), ("d_heights", C.c_void_p), ("stream", C.c_void_p),
-                ("device", C.c_int32), ("reserved", C.c_uint32)]
+                ("device", C.c_int32), ("lanes", C.c_uint32)]
 
 
 class RsosError(RuntimeError):
@@ -89,11 +89,11 @@ class Rsos:
     """
 
     def __init__(self, L, N, R, seed, tile=0, subsweeps=0, first_real=0, engine=ENGINE_AUTO,
-                 d_heights=None, stream=None, device=None):
+                 d_heights=None, stream=None, device=None, lanes=0):
         self._l = load()
         self.L, self.N, self.R, self.seed = int(L), int(N), int(R), int(seed)
         o = RsosOpts(int(tile), int(subsweeps), int(first_real), int(engine), d_heights or None,
-                     stream or None, 0 if device is None else int(device) + 1, 0)
+                     stream or None, 0 if device is None else int(device) + 1, int(lanes))
         self._c = C.c_void_p()
         _check(self._l.rsos_init(C.byref(self._c), self.L, self.N, self.R, self.seed, C.byref(o)))
 

@@ -36,54 +36,130 @@ struct TGeom {
     static constexpr uint32_t NTW = (TBITS + 31) / 32;             // words of one tile row
 };
 
-// One attempt at tile site (dx, dy) of this lane's tile; `base` = this lane's byte address of word
-// 0 in shared memory.  Returns 1 if the deposit was accepted (D:2 step 6; D:3 (i)).
-template <int LGS, int FB>
-__device__ __forceinline__ uint32_t thread_attempt(uint32_t base, uint32_t dx, uint32_t dy, uint32_t N)
-{
+// ---------------------------------------------------------------------------------------------
+// KL lanes share one tile (KL = 1, 2 or 4; 32 / KL tiles per warp).  In every step the KL lanes of a
+// group take KL consecutive attempts a0 + rank on the same snapshot of the tile.  A lane whose site
+// is equal or adjacent to the site of a LOWER rank of its group, or shares a byte of packed sites
+// with it, is "hazardous": it waits until the lower ranks have stored and then loads and decides
+// again (rank by rank).  All other lanes cannot be affected by any lower rank, so their snapshot
+// decision is the sequential one.  Stores are single bytes, so lanes that merely share a word do
+// not interfere.  KL > 1 buys thread-level parallelism when a pass has few tiles (D:4).
+// ---------------------------------------------------------------------------------------------
+template <int LGS, int FB, int KL>
+struct Attempt {
     using G = TGeom<LGS, FB>;
-    constexpr uint32_t M = G::M;
-    const uint32_t bl = dx * FB;                          // bit of the left neighbour (window column dx)
-    const uint32_t bc = bl + FB;                          // bit of the site itself (window column dx + 1)
-    const uint32_t row = base + (dy + 1u) * G::ROWB;
-    const uint32_t a0 = row + (bl >> 5) * 128u;           // word holding the left neighbour
-    const uint32_t ac = row + (bc >> 5) * 128u;           // word holding the site (and U/D columns)
+    static constexpr uint32_t NT = 32 / KL;               // tiles per warp = word stride (in words)
+    static constexpr uint32_t WSB = NT * 4;               // byte stride between consecutive words of a tile
+    static constexpr uint32_t ROWB = G::PW * WSB;         // byte stride between window rows
+    uint32_t a0, ac;      // shared-memory byte addresses: word of the left neighbour, word of the site
+    uint32_t sl, sc;      // bit positions of the left neighbour / the site inside those words
+    uint32_t key;         // dy * 128 + dx: sites are equal or adjacent iff keys differ by 0, 1 or 128
     uint32_t w0, w1, wu, wd;
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(w0) : "r"(a0));
-    asm volatile("ld.shared.u32 %0, [%1+128];" : "=r"(w1) : "r"(a0));
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(wu) : "r"(ac - G::ROWB));
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(wd) : "r"(ac + G::ROWB));
-    const uint32_t sc = bc & 31u;
-    const uint32_t t3 = __funnelshift_r(w0, w1, bl & 31u);        // fields: L, C, R (garbage above)
-    const uint32_t c = t3 >> FB;                                  // C in the low FB bits
-    // Under Eq. (6) the deposit is rejected iff some neighbour sits at h - N, i.e. (C - nb) mod 2^FB == N
-    // (D:3 (i)).  Branch-free: four independent subtract / test pairs.
-    const uint32_t okL = ((c - t3) ^ N) & M;
-    const uint32_t okR = ((c - (t3 >> (2 * FB))) ^ N) & M;
-    const uint32_t okU = ((c - (wu >> sc)) ^ N) & M;
-    const uint32_t okD = ((c - (wd >> sc)) ^ N) & M;
-    const bool ok = (okL != 0u) & (okR != 0u) & (okU != 0u) & (okD != 0u);
-    const uint32_t own = (bc >> 5) == (bl >> 5) ? w0 : w1;
-    const uint32_t nw = own ^ (((c ^ (c + 1u)) & M) << sc);       // field + 1 mod 2^FB
-    asm volatile("{ .reg .pred p; setp.ne.u32 p, %2, 0; @p st.shared.u32 [%0], %1; }"
-                 :: "r"(ac), "r"(nw), "r"((uint32_t)ok) : "memory");
+
+    // v: 16-bit slot, dx = v & (S-1), dy = (v >> LGS) & (S-1)   (D:2 step 6)
+    __device__ __forceinline__ void prep(uint32_t base, uint32_t v)
+    {
+        const uint32_t dx = v & (G::S - 1u), dy = (v >> LGS) & (G::S - 1u);
+        const uint32_t bl = dx * FB, bc = bl + FB;        // window columns dx (left neighbour) and dx + 1 (site)
+        const uint32_t row = base + (dy + 1u) * ROWB;
+        a0 = row + (bl >> 5) * WSB;
+        ac = row + (bc >> 5) * WSB;
+        sl = bl & 31u;
+        sc = bc & 31u;
+        key = dy * 128u + dx;
+    }
+    __device__ __forceinline__ void load()
+    {
+        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(w0) : "r"(a0));
+        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(w1) : "r"(a0 + WSB));
+        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(wu) : "r"(ac - ROWB));
+        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(wd) : "r"(ac + ROWB));
+    }
+    // Eq. (6) test on the loaded words: rejected iff some neighbour sits at h - N, i.e.
+    // (C - nb) mod 2^FB == N (D:3 (i)).  nw = the site's word with field C turned into C + 1 mod 2^FB.
+    __device__ __forceinline__ bool decide(uint32_t N, uint32_t &nw) const
+    {
+        constexpr uint32_t M = G::M;
+        const uint32_t t3 = __funnelshift_r(w0, w1, sl);           // fields: L, C, R (garbage above)
+        const uint32_t c = t3 >> FB;
+        const uint32_t okL = ((c - t3) ^ N) & M;
+        const uint32_t okR = ((c - (t3 >> (2 * FB))) ^ N) & M;
+        const uint32_t okU = ((c - (wu >> sc)) ^ N) & M;
+        const uint32_t okD = ((c - (wd >> sc)) ^ N) & M;
+        nw = (a0 == ac ? w0 : w1) ^ (((c ^ (c + 1u)) & M) << sc);
+        return (okL != 0u) & (okR != 0u) & (okU != 0u) & (okD != 0u);
+    }
+    __device__ __forceinline__ void store(uint32_t nw) const
+    {
+        if (KL == 1) {
+            asm volatile("st.shared.u32 [%0], %1;" :: "r"(ac), "r"(nw) : "memory");
+        } else {                                           // only the byte holding the site
+            asm volatile("st.shared.u8 [%0], %1;" :: "r"(ac + (sc >> 3)), "r"(nw >> (sc & 24u)) : "memory");
+        }
+    }
+};
+
+// One step: this lane's attempt (slot v).  Returns 1 if the deposit was accepted.
+template <int LGS, int FB, int KL>
+__device__ __forceinline__ uint32_t thread_step(uint32_t base, uint32_t v, uint32_t N, uint32_t rank)
+{
+    constexpr uint32_t FULL = 0xFFFFFFFFu;
+    Attempt<LGS, FB, KL> a;
+    a.prep(base, v);
+    a.load();
+    uint32_t nw;
+    bool ok = a.decide(N, nw);
+    if (KL == 1) {
+        if (ok) a.store(nw);
+        return ok ? 1u : 0u;
+    }
+    // hazard against the lower ranks of the group, from the site keys alone
+    bool hz = false;
+    const uint32_t bkey = (a.key + 1u) >> (FB == 2 ? 2 : 1);       // byte of packed sites holding the site
+#pragma unroll
+    for (int i = 1; i < KL; ++i) {
+        const uint32_t ko = __shfl_up_sync(FULL, a.key, i);
+        const int32_t d = (int32_t)(a.key - ko);
+        const uint32_t d2 = (uint32_t)(d * d);
+        const bool bad = (d2 <= 1u) | (d2 == 128u * 128u) | (((ko + 1u) >> (FB == 2 ? 2 : 1)) == bkey);
+        hz |= bad & ((uint32_t)i <= rank);
+    }
+    if (ok & !hz) a.store(nw);
+    __syncwarp();
+    if (__any_sync(FULL, hz)) {
+#pragma unroll
+        for (int rr = 1; rr < KL; ++rr) {
+            const bool mine = hz & (rank == (uint32_t)rr);
+            if (__any_sync(FULL, mine)) {
+                if (mine) {
+                    a.load();
+                    ok = a.decide(N, nw);
+                    if (ok) a.store(nw);
+                }
+                __syncwarp();
+            }
+        }
+    }
     return ok ? 1u : 0u;
 }
 
-// Block b runs tile set b: 32 active tiles, one per lane.
-template <int LGS, int FB>
+// Block b (one warp) runs tile set b: 32 / KL active tiles, KL lanes per tile.
+template <int LGS, int FB, int KL>
 __global__ void __launch_bounds__(32) thread_dt_kernel(Params p, uint32_t u, uint32_t colour)
 {
     using G = TGeom<LGS, FB>;
-    constexpr uint32_t S = G::S, PW = G::PW, NTW = G::NTW;
+    using At = Attempt<LGS, FB, KL>;
+    constexpr uint32_t S = G::S, PW = G::PW, NTW = G::NTW, NT = At::NT;
+    constexpr uint32_t FULL = 0xFFFFFFFFu;
     extern __shared__ __align__(16) uint32_t smem[];
     const uint32_t lane = threadIdx.x;
+    const uint32_t grp = lane / KL, rank = lane % KL;
     const uint32_t L = p.L, Lm = L - 1;
     const uint32_t T = L >> LGS, half = T >> 1, ntile = half * half;
     const uint32_t total = p.R * ntile;
-    uint32_t idx = blockIdx.x * 32u + lane;
+    uint32_t idx = blockIdx.x * NT + grp;
     const bool live = idx < total;
-    if (!live) idx = total - 1u;                         // idle lanes shadow the last tile, write nothing
+    if (!live) idx = total - 1u;                         // idle groups shadow the last tile, write nothing
     const uint32_t rl = idx / ntile, n = idx - rl * ntile;
     const uint32_t ti = n % half, tj = n / half;
     const uint32_t I = 2 * ti + (colour & 1u), J = 2 * tj + (colour >> 1);
@@ -93,7 +169,7 @@ __global__ void __launch_bounds__(32) thread_dt_kernel(Params p, uint32_t u, uin
     const uint32_t x0 = (ox + I * S) & Lm, y0 = (oy + J * S) & Lm;
     const uint32_t wpr = L >> G::LGSPW, wm = wpr - 1u;    // packed words per lattice row
     uint32_t *pk = p.pk + (size_t)rl * L * wpr;
-    uint32_t *my = smem + lane;                           // word w of this lane: my[w * 32]
+    uint32_t *my = smem + grp;                            // word w of this group's tile: my[w * NT]
     const uint32_t base = (uint32_t)__cvta_generic_to_shared(my);
 
     // ---- a3: stage rows y0-1 .. y0+S; window column X <-> lattice column x0 - 1 + X ------------
@@ -101,47 +177,60 @@ __global__ void __launch_bounds__(32) thread_dt_kernel(Params p, uint32_t u, uin
         const uint32_t gxs = (x0 - 1u) & Lm;
         const uint32_t ws = gxs >> G::LGSPW, o = (gxs & (G::SPW - 1u)) * FB;
 #pragma unroll 2
-        for (uint32_t yr = 0; yr < G::ROWS; ++yr) {
+        for (uint32_t yr = rank; yr < G::ROWS; yr += KL) {
             const uint32_t *rowp = pk + (size_t)((y0 - 1u + yr) & Lm) * wpr;
             uint32_t g[PW + 1];
 #pragma unroll
             for (uint32_t k = 0; k <= PW; ++k) g[k] = rowp[(ws + k) & wm];
 #pragma unroll
-            for (uint32_t k = 0; k < PW; ++k) my[(yr * PW + k) * 32u] = __funnelshift_r(g[k], g[k + 1], o);
+            for (uint32_t k = 0; k < PW; ++k) my[(yr * PW + k) * NT] = __funnelshift_r(g[k], g[k + 1], o);
         }
     }
     __syncwarp();
 
-    // ---- a1 + a4: A attempts in order; call q serves attempts 8q .. 8q+7 (16-bit slots) -------
+    // ---- a1 + a4: A attempts in order, KL per step.  Attempt a takes the 16-bit slot a & 7 of
+    // Philox call a >> 3 (D:2 step 6).  A batch is KL calls = 8 steps; rank r computes call
+    // batch * KL + r and the slots travel inside the group by shuffles.
     const uint32_t A = (S * S) / p.K;
     const uint32_t tile_id = J * T + I;
     const uint32_t N = p.N;
     uint32_t nacc = 0;
 #pragma unroll 1
-    for (uint32_t q = 0; q < A / 8u; ++q) {
-        const uint4 o = philox4x32_10(q, tile_id, u, rg, p.k0, p.k1);
+    for (uint32_t batch = 0; batch < A / (8u * KL); ++batch) {
+        const uint4 o = philox4x32_10(batch * KL + rank, tile_id, u, rg, p.k0, p.k1);
         const uint32_t ow[4] = {o.x, o.y, o.z, o.w};
 #pragma unroll
-        for (uint32_t j = 0; j < 8; ++j) {
-            const uint32_t v = (ow[j >> 1] >> (16u * (j & 1u))) & 0xFFFFu;
-            nacc += thread_attempt<LGS, FB>(base, v & (S - 1u), (v >> LGS) & (S - 1u), N);
+        for (uint32_t w = 0; w < 8; ++w) {
+            uint32_t v;
+            if (KL == 1) {
+                v = (ow[w >> 1] >> (16u * (w & 1u))) & 0xFFFFu;
+            } else if (KL == 2) {                         // attempt 2w + rank of the batch: call w >> 2, slot 2(w & 3) + rank
+                const uint32_t x = __shfl_sync(FULL, ow[w & 3u], grp * KL + (w >> 2));
+                v = rank ? x >> 16 : x & 0xFFFFu;
+            } else {                                      // KL == 4: attempt 4w + rank: call w >> 1, slot 4(w & 1) + rank
+                const uint32_t src = grp * KL + (w >> 1);
+                const uint32_t xa = __shfl_sync(FULL, ow[2u * (w & 1u)], src);
+                const uint32_t xb = __shfl_sync(FULL, ow[2u * (w & 1u) + 1u], src);
+                const uint32_t x = (rank & 2u) ? xb : xa;
+                v = (rank & 1u) ? x >> 16 : x & 0xFFFFu;
+            }
+            nacc += thread_step<LGS, FB, KL>(base, v, N, rank);
         }
     }
     __syncwarp();
-    if (!live) return;
 
     // ---- a5: write back the S x S tile bits.  A tile row is TBITS bits starting at bit ob of
     // packed word wsb; whole words are stored, the (at most two) partial edge words are merged
     // with the lattice word.  No other tile of this pass touches those words: tiles of one colour
     // are S >= SPW sites apart (D:5).
-    {
+    if (live) {
         const uint32_t wsb = x0 >> G::LGSPW, ob = (x0 & (G::SPW - 1u)) * FB;
 #pragma unroll 1
-        for (uint32_t Y = 1; Y <= S; ++Y) {
+        for (uint32_t Y = 1u + rank; Y <= S; Y += KL) {
             uint32_t *rowp = pk + (size_t)((y0 - 1u + Y) & Lm) * wpr;
             uint32_t w[PW + 1];
 #pragma unroll
-            for (uint32_t k = 0; k < PW; ++k) w[k] = my[(Y * PW + k) * 32u];
+            for (uint32_t k = 0; k < PW; ++k) w[k] = my[(Y * PW + k) * NT];
             w[PW] = 0u;
             uint32_t tb[NTW + 2], tm[NTW + 2];             // tile bits / valid mask, padded with a zero word each side
             tb[0] = 0u; tm[0] = 0u; tb[NTW + 1] = 0u; tm[NTW + 1] = 0u;
@@ -161,23 +250,35 @@ __global__ void __launch_bounds__(32) thread_dt_kernel(Params p, uint32_t u, uin
                 else if (mk != 0u) *dst = (*dst & ~mk) | gk;
             }
         }
+        if (nacc) atomicAdd(p.accepted + rl, (unsigned long long)nacc);
     }
-    if (nacc) atomicAdd(p.accepted + rl, (unsigned long long)nacc);
 }
 
 // =============================================================================================
 // Host-side launchers
 // =============================================================================================
-template <int LGS, int FB>
+template <int LGS, int FB, int KL>
 static cudaError_t thread_dt_t(const Params &p, uint32_t u, uint32_t colour, uint32_t blocks, cudaStream_t st, int what,
                                size_t *out)
 {
-    const size_t sm = (size_t)32 * TGeom<LGS, FB>::WORDS * 4;
+    const size_t sm = (size_t)(32 / KL) * TGeom<LGS, FB>::WORDS * 4;
     if (what == 0) { *out = sm; return cudaSuccess; }
     if (what == 1)
-        return cudaFuncSetAttribute(thread_dt_kernel<LGS, FB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    thread_dt_kernel<LGS, FB><<<blocks, 32, sm, st>>>(p, u, colour);
+        return cudaFuncSetAttribute(thread_dt_kernel<LGS, FB, KL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    thread_dt_kernel<LGS, FB, KL><<<blocks, 32, sm, st>>>(p, u, colour);
     return cudaGetLastError();
+}
+
+template <int LGS, int FB>
+static cudaError_t thread_dt_k(const Params &p, uint32_t u, uint32_t colour, uint32_t blocks, cudaStream_t st, int what,
+                               size_t *out)
+{
+    switch (p.KL) {
+        case 1: return thread_dt_t<LGS, FB, 1>(p, u, colour, blocks, st, what, out);
+        case 2: return thread_dt_t<LGS, FB, 2>(p, u, colour, blocks, st, what, out);
+        case 4: return thread_dt_t<LGS, FB, 4>(p, u, colour, blocks, st, what, out);
+        default: return cudaErrorInvalidValue;
+    }
 }
 
 static cudaError_t thread_dispatch(const Params &p, uint32_t u, uint32_t colour, uint32_t blocks, cudaStream_t st,
@@ -185,13 +286,13 @@ static cudaError_t thread_dispatch(const Params &p, uint32_t u, uint32_t colour,
 {
     const bool two = p.FB == 2;
     switch (p.lgS) {
-        case 3: return thread_dt_t<3, 4>(p, u, colour, blocks, st, what, out);      // S = 8 < 16 sites per 2-bit word
-        case 4: return two ? thread_dt_t<4, 2>(p, u, colour, blocks, st, what, out)
-                           : thread_dt_t<4, 4>(p, u, colour, blocks, st, what, out);
-        case 5: return two ? thread_dt_t<5, 2>(p, u, colour, blocks, st, what, out)
-                           : thread_dt_t<5, 4>(p, u, colour, blocks, st, what, out);
-        case 6: return two ? thread_dt_t<6, 2>(p, u, colour, blocks, st, what, out)
-                           : thread_dt_t<6, 4>(p, u, colour, blocks, st, what, out);
+        case 3: return thread_dt_k<3, 4>(p, u, colour, blocks, st, what, out);      // S = 8 < 16 sites per 2-bit word
+        case 4: return two ? thread_dt_k<4, 2>(p, u, colour, blocks, st, what, out)
+                           : thread_dt_k<4, 4>(p, u, colour, blocks, st, what, out);
+        case 5: return two ? thread_dt_k<5, 2>(p, u, colour, blocks, st, what, out)
+                           : thread_dt_k<5, 4>(p, u, colour, blocks, st, what, out);
+        case 6: return two ? thread_dt_k<6, 2>(p, u, colour, blocks, st, what, out)
+                           : thread_dt_k<6, 4>(p, u, colour, blocks, st, what, out);
         default: return cudaErrorInvalidValue;
     }
 }
@@ -199,6 +300,15 @@ static cudaError_t thread_dispatch(const Params &p, uint32_t u, uint32_t colour,
 // Field width of the packed lattice (D:5): 2 bits when N = 1 and a tile is at least one 2-bit
 // word wide (so that tiles of one colour never share a packed word), else 4 bits (N <= 7).
 uint32_t thread_dt_field_bits(uint32_t N, uint32_t S) { return (N <= 1u && S >= 16u) ? 2u : 4u; }
+
+// Lanes per tile (D:4): the fewest that still give every SM sub-partition about two warps.
+uint32_t thread_dt_lanes_per_tile(uint64_t pass_tiles, int sm_count)
+{
+    const uint64_t want_warps = (uint64_t)sm_count * 4 * 2;
+    for (uint32_t kl = 1; kl < 4; kl *= 2)
+        if (pass_tiles * kl / 32 >= want_warps) return kl;
+    return 4;
+}
 
 size_t thread_dt_smem(const Params &p)
 {
@@ -213,7 +323,8 @@ uint32_t thread_dt_blocks(const Params &p)
 {
     const uint32_t T = p.L >> p.lgS, half = T >> 1;
     const uint64_t tiles = (uint64_t)p.R * half * half;
-    return (uint32_t)((tiles + 31) / 32);
+    const uint32_t nt = 32u / p.KL;
+    return (uint32_t)((tiles + nt - 1) / nt);
 }
 
 cudaError_t thread_dt_launch(const Params &p, uint32_t u, uint32_t colour, uint32_t blocks, cudaStream_t st)

@@ -101,9 +101,10 @@ def test_dt_warp_engine_equals_oracle(rsos, oracle_mod, L, N, R, S, K, mcs, seed
     (64, 1, 2, 8, 2, 5, 8),          # S = 8, A = 32 attempts per tile
     (128, 1, 1, 64, 128, 2, 11),     # A = 32
 ])
-def test_dt_thread_engine_equals_oracle(rsos, oracle_mod, L, N, R, S, K, mcs, seed):
-    """The lane-per-tile engine (2- or 4-bit sites, bank-interleaved shared memory)."""
-    g = rsos.Rsos(L, N, R, seed, tile=S, subsweeps=K, engine=rsos.ENGINE_THREAD)
+@pytest.mark.parametrize("lanes", [1, 2, 4])
+def test_dt_thread_engine_equals_oracle(rsos, oracle_mod, L, N, R, S, K, mcs, seed, lanes):
+    """The lane-per-tile engine (2- or 4-bit sites, bank-interleaved shared memory), 1, 2 or 4 lanes per tile."""
+    g = rsos.Rsos(L, N, R, seed, tile=S, subsweeps=K, engine=rsos.ENGINE_THREAD, lanes=lanes)
     o = oracle_mod.Oracle(L, N, R, seed, tile=S, subsweeps=K)
     assert g.info()["mode"] == "DT" and g.info()["engine"] == "thread"
     for step in range(mcs):
@@ -116,9 +117,10 @@ def test_dt_thread_engine_equals_oracle(rsos, oracle_mod, L, N, R, S, K, mcs, se
 @pytest.mark.parametrize("L,N,R,mcs", [(2048, 1, 2, 2),     # 512 tiles per pass; rows rebuilt by one warp each
                                        (4096, 1, 1, 1),     # 256 packed words per row: rows rebuilt by a whole block
                                        (2048, 3, 1, 1)])    # 4-bit sites, 256 words per row
-def test_dt_thread_engine_large_lattices(rsos, oracle_mod, L, N, R, mcs):
+@pytest.mark.parametrize("lanes", [0, 2])
+def test_dt_thread_engine_large_lattices(rsos, oracle_mod, L, N, R, mcs, lanes):
     """Many tiles per pass and both row-team shapes of the packed -> int32 rebuild (rsos_pack.cu)."""
-    g = rsos.Rsos(L, N, R, 13, engine=rsos.ENGINE_THREAD)
+    g = rsos.Rsos(L, N, R, 13, engine=rsos.ENGINE_THREAD, lanes=lanes)
     o = oracle_mod.Oracle(L, N, R, 13)
     g.advance(mcs)
     o.advance(mcs)
