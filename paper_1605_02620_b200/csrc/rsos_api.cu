@@ -32,7 +32,8 @@ struct rsos_ctx {
     bool h_valid, pk_valid;           // which of the two copies is current (both after init)
     long long *d_s1off;               // R int64: sum h = s1off + accepted while pk is the current copy
     int32_t *d_V;                     // R * L int32 scratch (column chain)
-    unsigned long long *d_srel;       // R uint64 scratch
+    unsigned long long *d_srel;       // 4R uint64 scratch (sum rel, sum rel^2, min rel, max rel)
+    unsigned long long *h_pk;         // pinned host mirror: 4R (d_srel) + R (s1off) uint64
     int32_t *d_h00;                   // R int32 scratch
     size_t smem_bytes;
     // optional timing of rsos_advance
@@ -90,6 +91,7 @@ static void destroy(rsos_ctx *c)
     if (c->d_s1off) cudaFree(c->d_s1off);
     if (c->d_V) cudaFree(c->d_V);
     if (c->d_srel) cudaFree(c->d_srel);
+    if (c->h_pk) cudaFreeHost(c->h_pk);
     if (c->d_h00) cudaFree(c->d_h00);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
@@ -189,7 +191,8 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
         INIT_TRY(cudaMalloc(&p.pk, pk_bytes), RSOS_ECUDA);
         INIT_TRY(cudaMalloc(&c->d_s1off, (size_t)R * sizeof(long long)), RSOS_ECUDA);
         INIT_TRY(cudaMalloc(&c->d_V, (size_t)R * L * sizeof(int32_t)), RSOS_ECUDA);
-        INIT_TRY(cudaMalloc(&c->d_srel, (size_t)R * sizeof(unsigned long long)), RSOS_ECUDA);
+        INIT_TRY(cudaMalloc(&c->d_srel, (size_t)R * 4 * sizeof(unsigned long long)), RSOS_ECUDA);
+        INIT_TRY(cudaMallocHost(&c->h_pk, (size_t)R * 5 * sizeof(unsigned long long)), RSOS_ECUDA);
         INIT_TRY(cudaMalloc(&c->d_h00, (size_t)R * sizeof(int32_t)), RSOS_ECUDA);
         INIT_TRY(cudaMemsetAsync(p.pk, 0, pk_bytes, c->stream), RSOS_ECUDA);                // flat start
         INIT_TRY(cudaMemsetAsync(c->d_s1off, 0, (size_t)R * sizeof(long long), c->stream), RSOS_ECUDA);
@@ -305,20 +308,58 @@ static int check_device_err(rsos_ctx *c)
     return RSOS_OK;
 }
 
+// THREAD engine, packed lattice current: S1, S2 and max |h| straight from the packed lattice
+// (rsos_pack.cu): h = h00 + rel with h00 = (S1 - sum rel) / L^2 and S1 = s1off + accepted, so
+// S2 = sum rel^2 + 2 h00 sum rel + L^2 h00^2.  All exact (128-bit on the host).
+static int reduce_sums_packed(rsos_ctx *c)
+{
+    const Params &p = c->p;
+    const size_t R = p.R;
+    CUDA_TRY(launch_packed_sums(p, c->d_V, c->d_srel, c->stream));
+    c->launches += 3;
+    CUDA_TRY(cudaMemcpyAsync(c->h_pk, c->d_srel, R * 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaMemcpyAsync(c->h_pk + R * 4, c->d_s1off, R * sizeof(long long), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaMemcpyAsync(c->h_red + R * 4, p.accepted, R * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+    const int rc = check_device_err(c);
+    if (rc) return rc;
+    const __int128 n = (__int128)p.L * p.L;
+    for (size_t r = 0; r < R; ++r) {
+        const long long srel = (long long)c->h_pk[4 * r], mn = (long long)c->h_pk[4 * r + 2], mx = (long long)c->h_pk[4 * r + 3];
+        const unsigned long long srel2 = c->h_pk[4 * r + 1];
+        const long long s1 = (long long)c->h_pk[4 * R + r] + (long long)c->h_red[4 * R + r];
+        const long long num = s1 - srel;
+        const long long h00 = num >> (2 * p.lgL);
+        if ((h00 << (2 * p.lgL)) != num)
+            return fail(RSOS_ECUDA, "realization %zu: packed lattice is inconsistent with sum h (reconstruction not exact)", r);
+        const long long lo = h00 + mn, hi = h00 + mx;
+        const unsigned long long amax = (unsigned long long)((lo < 0 ? -lo : lo) > (hi < 0 ? -hi : hi) ? (lo < 0 ? -lo : lo)
+                                                                                                     : (hi < 0 ? -hi : hi));
+        const __int128 s2 = (__int128)srel2 + 2 * (__int128)h00 * srel + n * (__int128)h00 * h00;
+        if (amax > 0x7FFFFFFFull || s2 < 0 || (s2 >> 64) != 0)
+            return fail(RSOS_ERANGE, "realization %zu: max|h| = %llu makes sum h^2 overflow 64 bits", r, amax);
+        c->h_red[4 * r] = (unsigned long long)s1;
+        c->h_red[4 * r + 1] = (unsigned long long)s2;
+        c->h_red[4 * r + 2] = amax;
+    }
+    return RSOS_OK;
+}
+
 static int reduce_sums(rsos_ctx *c)
 {
     const Params &p = c->p;
-    {
-        const int rc0 = ensure_heights(c);
+    if (p.pk && !c->h_valid) {
+        const int rc0 = reduce_sums_packed(c);
         if (rc0) return rc0;
+    } else {
+        CUDA_TRY(launch_sums(p.h, p.L, p.R, c->d_red, c->stream));
+        c->launches += (p.R + 65534) / 65535;
+        CUDA_TRY(cudaMemcpyAsync(c->h_red, c->d_red, (size_t)p.R * 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost,
+                                 c->stream));
+        CUDA_TRY(cudaMemcpyAsync(c->h_red + (size_t)p.R * 4, p.accepted, (size_t)p.R * sizeof(unsigned long long),
+                                 cudaMemcpyDeviceToHost, c->stream));
+        const int rc = check_device_err(c);
+        if (rc) return rc;
     }
-    CUDA_TRY(launch_sums(p.h, p.L, p.R, c->d_red, c->stream));
-    c->launches += (p.R + 65534) / 65535;
-    CUDA_TRY(cudaMemcpyAsync(c->h_red, c->d_red, (size_t)p.R * 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
-    CUDA_TRY(cudaMemcpyAsync(c->h_red + (size_t)p.R * 4, p.accepted, (size_t)p.R * sizeof(unsigned long long),
-                             cudaMemcpyDeviceToHost, c->stream));
-    int rc = check_device_err(c);
-    if (rc) return rc;
     // sum h^2 must stay below 2^64: max|h|^2 * L^2 < 2^64
     for (uint32_t r = 0; r < p.R; ++r) {
         const unsigned __int128 mx = c->h_red[4 * (size_t)r + 2];
@@ -372,7 +413,9 @@ extern "C" int rsos_moments(rsos_ctx *c, int64_t *base, uint64_t *out)
     if (!out) return fail(RSOS_EINVAL, "out is NULL");
     DeviceGuard guard(c->device);
     if (!guard.ok) return fail(RSOS_ECUDA, "cannot select CUDA device %d", c->device);
-    int rc = reduce_sums(c);
+    int rc = ensure_heights(c);                            // the moment kernel reads the int32 heights
+    if (rc) return rc;
+    rc = reduce_sums(c);
     if (rc) return rc;
     const Params &p = c->p;
     long long *hb = reinterpret_cast<long long *>(c->h_red + (size_t)p.R * 5);

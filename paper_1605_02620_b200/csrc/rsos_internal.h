@@ -34,6 +34,7 @@ cudaError_t thread_dt_launch(const Params &p, uint32_t u, uint32_t colour, uint3
 // rsos_pack.cu (packed working lattice <-> int32 heights)
 cudaError_t launch_pack(const Params &p, cudaStream_t st);
 cudaError_t launch_s1off(const Params &p, const unsigned long long *d_red, long long *d_s1off, cudaStream_t st);
+cudaError_t launch_packed_sums(const Params &p, int32_t *d_V, unsigned long long *d_srel, cudaStream_t st);
 cudaError_t launch_unpack(const Params &p, const long long *d_s1off, int32_t *d_V, unsigned long long *d_srel,
                           int32_t *d_h00, cudaStream_t st, uint32_t *launches);
 

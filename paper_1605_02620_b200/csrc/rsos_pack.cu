@@ -109,7 +109,8 @@ __global__ void __launch_bounds__(256) unpack_col_kernel(const uint32_t *__restr
 // wpr >= 256, else one warp (8 rows per block).  Every thread owns a contiguous run of words,
 // sums its differences, the team scans the totals, and a second sweep over the same words forms
 // rel(x, y) = V(y) + H(x, y) site by site.
-//   WRITE = false: srel[r] += sum_x rel(x, y)                 (exact, int64)
+//   WRITE = false: srel[4r + 0] += sum_x rel, srel[4r + 1] += sum_x rel^2 (exact, 64-bit),
+//                  srel[4r + 2] = min rel, srel[4r + 3] = max rel (signed 64-bit)
 //   WRITE = true : h[r][y][x] = h00[r] + rel(x, y)            (int4 stores)
 // ---------------------------------------------------------------------------------------------
 template <int FB, bool WRITE>
@@ -164,6 +165,8 @@ __global__ void __launch_bounds__(256) unpack_rows_kernel(const uint32_t *__rest
     if (row_ok) run += V[row];
     if (WRITE && row_ok) run += h00[rl];
     long long acc = 0;
+    unsigned long long acc2 = 0;
+    int32_t mn = 0x7FFFFFFF, mx = -0x7FFFFFFF - 1;
     {
         uint32_t pf = prevf;
         for (uint32_t i = 0; i < nw; ++i) {
@@ -175,7 +178,12 @@ __global__ void __launch_bounds__(256) unpack_rows_kernel(const uint32_t *__rest
                 run += sdiff<FB>(f, pf);
                 pf = f;
                 out[k] = run;
-                if (!WRITE) acc += run;
+                if (!WRITE) {
+                    acc += run;
+                    acc2 += (unsigned long long)((long long)run * run);
+                    mn = min(mn, run);
+                    mx = max(mx, run);
+                }
             }
             if (WRITE) {
                 int4 *dst = reinterpret_cast<int4 *>(h + (size_t)row * L + (size_t)(w0 + i) * SPW);
@@ -187,18 +195,41 @@ __global__ void __launch_bounds__(256) unpack_rows_kernel(const uint32_t *__rest
     }
     if (!WRITE) {
 #pragma unroll
-        for (int o = 16; o; o >>= 1) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
-        if (lane == 0 && row_ok && acc != 0) atomicAdd(srel + rl, (unsigned long long)acc);
+        for (int o = 16; o; o >>= 1) {
+            acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
+            acc2 += __shfl_xor_sync(0xFFFFFFFFu, acc2, o);
+            mn = min(mn, __shfl_xor_sync(0xFFFFFFFFu, mn, o));
+            mx = max(mx, __shfl_xor_sync(0xFFFFFFFFu, mx, o));
+        }
+        if (lane == 0 && row_ok) {
+            unsigned long long *d = srel + 4 * (size_t)rl;
+            if (acc != 0) atomicAdd(d, (unsigned long long)acc);
+            if (acc2 != 0) atomicAdd(d + 1, acc2);
+            if (mn <= mx) {
+                atomicMin(reinterpret_cast<long long *>(d + 2), (long long)mn);
+                atomicMax(reinterpret_cast<long long *>(d + 3), (long long)mx);
+            }
+        }
     }
 }
 
-// h00[r] = (s1off[r] + accepted[r] - srel[r]) / L^2, which must divide exactly and fit int32.
+__global__ void srel_init_kernel(unsigned long long *srel, uint32_t R)
+{
+    const uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= R) return;
+    srel[4 * (size_t)r] = 0ull;
+    srel[4 * (size_t)r + 1] = 0ull;
+    srel[4 * (size_t)r + 2] = (unsigned long long)0x7FFFFFFFFFFFFFFFll;
+    srel[4 * (size_t)r + 3] = (unsigned long long)(-0x7FFFFFFFFFFFFFFFll - 1);
+}
+
+// h00[r] = (s1off[r] + accepted[r] - srel[4r]) / L^2, which must divide exactly and fit int32.
 __global__ void anchor_kernel(const long long *s1off, const unsigned long long *accepted, const unsigned long long *srel,
                               int32_t *h00, uint32_t lgL2, uint32_t R, uint32_t *err)
 {
     const uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= R) return;
-    const long long num = s1off[r] + (long long)accepted[r] - (long long)srel[r];
+    const long long num = s1off[r] + (long long)accepted[r] - (long long)srel[4 * (size_t)r];
     const long long q = num >> lgL2;
     if ((q << lgL2) != num || q > 0x7FFFFFFFll || q < -0x80000000ll) atomicOr(err, ERR_RECONSTRUCT);
     h00[r] = (int32_t)q;
@@ -222,7 +253,26 @@ cudaError_t launch_s1off(const Params &p, const unsigned long long *d_red, long 
     return cudaGetLastError();
 }
 
-// packed -> int32 heights of all realizations.  Scratch: d_V (R*L int32), d_srel (R uint64),
+// Sums of the relative heights straight from the packed lattice: d_srel[4r..4r+3] = sum rel,
+// sum rel^2, min rel, max rel (rel = h - h(0,0)).  Enough for S1, S2 and max |h| without
+// materialising the int32 heights.  Scratch: d_V (R*L int32).  3 kernels.
+cudaError_t launch_packed_sums(const Params &p, int32_t *d_V, unsigned long long *d_srel, cudaStream_t st)
+{
+    const uint32_t wpr = p.L * p.FB / 32;
+    const uint32_t nrows = p.R * p.L;
+    const uint32_t rblocks = wpr >= 256u ? nrows : (nrows + 7u) / 8u;
+    srel_init_kernel<<<(p.R + 127) / 128, 128, 0, st>>>(d_srel, p.R);
+    if (p.FB == 2) {
+        unpack_col_kernel<2><<<p.R, 256, 0, st>>>(p.pk, d_V, p.L, wpr);
+        unpack_rows_kernel<2, false><<<rblocks, 256, 0, st>>>(p.pk, d_V, nullptr, p.h, d_srel, p.L, wpr, nrows);
+    } else {
+        unpack_col_kernel<4><<<p.R, 256, 0, st>>>(p.pk, d_V, p.L, wpr);
+        unpack_rows_kernel<4, false><<<rblocks, 256, 0, st>>>(p.pk, d_V, nullptr, p.h, d_srel, p.L, wpr, nrows);
+    }
+    return cudaGetLastError();
+}
+
+// packed -> int32 heights of all realizations.  Scratch: d_V (R*L int32), d_srel (4R uint64),
 // d_h00 (R int32).  Returns the number of kernels launched through *launches.
 cudaError_t launch_unpack(const Params &p, const long long *d_s1off, int32_t *d_V, unsigned long long *d_srel,
                           int32_t *d_h00, cudaStream_t st, uint32_t *launches)
@@ -230,19 +280,12 @@ cudaError_t launch_unpack(const Params &p, const long long *d_s1off, int32_t *d_
     const uint32_t wpr = p.L * p.FB / 32;
     const uint32_t nrows = p.R * p.L;
     const uint32_t rblocks = wpr >= 256u ? nrows : (nrows + 7u) / 8u;
-    cudaError_t e = cudaMemsetAsync(d_srel, 0, (size_t)p.R * sizeof(unsigned long long), st);
+    cudaError_t e = launch_packed_sums(p, d_V, d_srel, st);
     if (e != cudaSuccess) return e;
-    if (p.FB == 2) {
-        unpack_col_kernel<2><<<p.R, 256, 0, st>>>(p.pk, d_V, p.L, wpr);
-        unpack_rows_kernel<2, false><<<rblocks, 256, 0, st>>>(p.pk, d_V, d_h00, p.h, d_srel, p.L, wpr, nrows);
-    } else {
-        unpack_col_kernel<4><<<p.R, 256, 0, st>>>(p.pk, d_V, p.L, wpr);
-        unpack_rows_kernel<4, false><<<rblocks, 256, 0, st>>>(p.pk, d_V, d_h00, p.h, d_srel, p.L, wpr, nrows);
-    }
     anchor_kernel<<<(p.R + 127) / 128, 128, 0, st>>>(d_s1off, p.accepted, d_srel, d_h00, 2 * p.lgL, p.R, p.err);
     if (p.FB == 2) unpack_rows_kernel<2, true><<<rblocks, 256, 0, st>>>(p.pk, d_V, d_h00, p.h, d_srel, p.L, wpr, nrows);
     else unpack_rows_kernel<4, true><<<rblocks, 256, 0, st>>>(p.pk, d_V, d_h00, p.h, d_srel, p.L, wpr, nrows);
-    *launches = 4;
+    *launches = 5;
     return cudaGetLastError();
 }
 
