@@ -113,15 +113,16 @@ __device__ __forceinline__ uint32_t thread_step(uint32_t base, uint32_t v, uint3
         if (ok) a.store(nw);
         return ok ? 1u : 0u;
     }
-    // hazard against the lower ranks of the group, from the site keys alone
+    // Hazard against the lower ranks of the group, from the site keys alone (key = dy * 128 + dx).
+    // Equal or adjacent sites have |d| in {0, 1, 128}; sites in one byte of packed sites lie in one
+    // row within 3 (2-bit) or 1 (4-bit) columns.  The test |d| <= 3 or |d| == 128 covers both and is
+    // conservative: a false alarm only costs a reload.
     bool hz = false;
-    const uint32_t bkey = (a.key + 1u) >> (FB == 2 ? 2 : 1);       // byte of packed sites holding the site
 #pragma unroll
     for (int i = 1; i < KL; ++i) {
         const uint32_t ko = __shfl_up_sync(FULL, a.key, i);
-        const int32_t d = (int32_t)(a.key - ko);
-        const uint32_t d2 = (uint32_t)(d * d);
-        const bool bad = (d2 <= 1u) | (d2 == 128u * 128u) | (((ko + 1u) >> (FB == 2 ? 2 : 1)) == bkey);
+        const uint32_t d = a.key - ko;
+        const bool bad = (d + 3u <= 6u) | (d == 128u) | (d == 0u - 128u);
         hz |= bad & ((uint32_t)i <= rank);
     }
     if (ok & !hz) a.store(nw);
@@ -247,7 +248,10 @@ __global__ void __launch_bounds__(32) thread_dt_kernel(Params p, uint32_t u, uin
                 const uint32_t mk = __funnelshift_l(tm[k], tm[k + 1], ob);
                 uint32_t *dst = rowp + ((wsb + k) & wm);
                 if (mk == 0xFFFFFFFFu) *dst = gk;
-                else if (mk != 0u) *dst = (*dst & ~mk) | gk;
+                else if (mk != 0u) {                        // partial word: clear my bits, then set them (no
+                    atomicAnd(dst, ~mk);                    // load to wait for; nobody else writes this word
+                    atomicOr(dst, gk);                      // in this pass and nobody reads my bits)
+                }
             }
         }
         if (nacc) atomicAdd(p.accepted + rl, (unsigned long long)nacc);
