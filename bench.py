@@ -70,15 +70,38 @@ def workload(args):
     return c
 
 
-def config_dict(args, c, n_gpus):
+def l2_note(c, info):
+    """Timing rule: say whether the inputs exceed L2 or are flushed.  A step sweeps the same resident lattice
+    mcs_per_step * 4K times, exactly as a production run does, so nothing is flushed; what is resident is stated."""
+    int32_mib = c["R"] * c["L"] ** 2 * 4 / 2 ** 20
+    if info and info.get("engine") == "thread":
+        fb = 2 if (c["N"] <= 1 and c["tile"] >= 16) else 4
+        work = int32_mib * fb / 32
+        return ("working lattice %.0f MiB per GPU (%d bits/site, DESIGN.md section 5; int32 view %.0f MiB) vs 126 MB L2: %s; "
+                "no flush: consecutive sweeps of a production run see the same residency" % (
+                    work, fb, int32_mib, "larger than L2" if work * 2 ** 20 > 126e6 else "L2-resident by design"))
+    return "state %.0f MiB int32 per GPU vs 126 MB L2: %s" % (
+        int32_mib, "inputs larger than L2, no flush" if int32_mib * 2 ** 20 > 2 * 126e6 else "L2/on-chip resident by design")
+
+
+def traffic_note(workload_name, info):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full summary (profiles/), or None."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        with open(path) as f:
+            t = json.load(f)
+        return t.get("%s/%s/lanes%d" % (workload_name, info["engine"], info.get("lanes", 0)))
+    except (OSError, ValueError):
+        return None
+
+
+def config_dict(args, c, n_gpus, info=None):
     mode = "RS" if 2 * c["tile"] > c["L"] else "DT(%d,%d)" % (c["tile"], c["subsweeps"])
     return {"workload": "%s: RSOS N=%d, L=%d periodic, %d realizations per GPU, int32 heights, flat start, seed %d"
                         % (args.workload, c["N"], c["L"], c["R"], c["seed"]),
             "schedule": mode, "mcs_per_step": c["mcs_per_step"],
             "step": "rsos_advance(mcs_per_step) + rsos_width",
-            "l2": "state %d MiB per GPU vs 126 MB L2: %s" % (
-                c["R"] * c["L"] ** 2 * 4 >> 20,
-                "inputs larger than L2, no flush" if c["R"] * c["L"] ** 2 * 4 > 2 * 126e6 else "L2/on-chip resident by design"),
+            "l2": l2_note(c, info),
             "parallelism": "replicas x%d (independent realizations, no collective)" % n_gpus}
 
 
@@ -302,9 +325,10 @@ def run_b200(args):
     avg_ms = upd_ms / max(1, upd_launches)
     achieved = per_launch_att * BYTES_PER_ATTEMPT / (avg_ms * 1e-3) / 1e9
     sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
-    alu_bound = info["sm_count"] * 32 * sm_mhz * 1e6 / 6.0          # 6 shared-memory ops / attempt
+    # issue bound = SMs x 4 schedulers x 32 lanes x measured SM clock / 22 instructions per attempt
+    alu_bound = info["sm_count"] * 4 * 32 * sm_mhz * 1e6 / 22.0
     roofline = {"bound": "hbm", "achieved": achieved, "peak": hbm, "unit": "GB/s", "frac": achieved / hbm,
-                "traffic": None, "peak_source": how, "kernel": "update kernel, engine=%s" % info["engine"],
+                "traffic": traffic_note(args.workload, info), "peak_source": how, "kernel": "update kernel, engine=%s" % info["engine"],
                 "bytes_per_attempt": BYTES_PER_ATTEMPT, "attempts_per_launch": per_launch_att,
                 "avg_launch_ms": avg_ms, "update_share_of_step": upd_ms / ms,
                 "alu_bound_attempts_per_s": alu_bound, "frac_of_alu_bound": (att_step * args.steps / (upd_ms * 1e-3)) / alu_bound,
@@ -317,7 +341,7 @@ def run_b200(args):
 
     line = {"metric": METRIC, "value": value / 1e9, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "int32", "data": "synthetic", "config": config_dict(args, c, world),
+            "vs_baseline": None, "dtype": "int32", "data": "synthetic", "config": config_dict(args, c, world, info),
             "engine": info, "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
             "cpu_baseline": cpu, "result_check": {"W2_mean": float(np.mean(W2)), "hmean_mean": float(np.mean(hmean)),
                                                   "t_mcs": int(g.t)}}

@@ -3,7 +3,7 @@
  * deposition Monte Carlo of arXiv 1605.02620 (Kelling, Odor, Gemming).
  *
  * Citations:  P:n = /root/reference/PAPER.md line n;  D:x = DESIGN.md section x (the seeded
- * schedule DT(S,K) / RS restated from SURVEY.md 8(c).1, and the readings Q1..Q15 of the paper).
+ * schedule DT(S,K) / RS restated from SURVEY.md 8(c).1, and the readings Q1..Q16 of the paper).
  *
  * What the library computes (Eq. 6): on a periodic L x L integer height lattice a site x
  * is picked at random and h(x) += 1 is accepted iff afterwards |h(x) - h(x')| <= N for the four
@@ -75,6 +75,9 @@ typedef struct rsos_opts {
     int32_t *d_heights;   /* DEVICE: borrowed buffer of R*L*L int32 (h[r][y][x], row-major, 16-   */
                           /* byte aligned), e.g. a torch tensor; NULL = the library allocates.    */
                           /* Its content on entry is ignored: rsos_init zeroes it (flat start).   */
+                          /* With the THREAD engine the working state is a packed lattice (D:5)   */
+                          /* and this buffer is brought up to date only by rsos_get_heights,      */
+                          /* rsos_moments, rsos_set_state and rsos_device_heights.                */
     void    *stream;      /* cudaStream_t to enqueue on; NULL = the legacy default stream         */
     int32_t  device;      /* CUDA device ordinal + 1; 0 = the current device                      */
     uint32_t lanes;       /* THREAD engine: lanes that share one tile, 1, 2 or 4; 0 = chosen from the     */
@@ -148,13 +151,17 @@ int rsos_time(rsos_ctx *ctx, uint64_t *t);
  * rsos_info -- describe the context: out[0] = mode (0 RS, 1 DT), out[1] = engine in use,
  * out[2] = S (effective tile side), out[3] = K, out[4] = kernel launches enqueued so far,
  * out[5] = device SM count, out[6] = shared-memory bytes per block of the update kernel,
- * out[7] = update-kernel blocks per launch.  Host buffer of 8 uint64.
+ * out[7] = update-kernel blocks per launch, out[8] = THREAD engine lanes per tile (else 0),
+ * out[9] = bits per site of the packed working lattice (THREAD engine, else 0).
+ * Host buffer of 10 uint64.
  */
 int rsos_info(rsos_ctx *ctx, uint64_t *out);
 
 /*
- * rsos_device_heights -- *d = the DEVICE pointer of the height buffer (borrowed or owned), valid
- * until rsos_free; reads of it must be ordered after the context's stream.
+ * rsos_device_heights -- *d = the DEVICE pointer of the int32 height buffer (borrowed or owned),
+ * valid until rsos_free.  The call first brings the buffer up to date on the context's stream
+ * (THREAD engine: rebuilt from the packed working lattice, D:5); its content is current as of this
+ * call and goes stale with the next rsos_advance.  Reads must be ordered after the stream.
  */
 int rsos_device_heights(rsos_ctx *ctx, int32_t **d);
 

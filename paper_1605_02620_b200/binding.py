@@ -161,10 +161,11 @@ class Rsos:
         return t.value
 
     def info(self):
-        a = (C.c_uint64 * 8)()
+        a = (C.c_uint64 * 10)()
         _check(self._l.rsos_info(self._c, a))
         return {"mode": "DT" if a[0] else "RS", "engine": ENGINE_NAMES[a[1]], "S": a[2], "K": a[3],
-                "launches": a[4], "sm_count": a[5], "smem_bytes": a[6], "blocks": a[7]}
+                "launches": a[4], "sm_count": a[5], "smem_bytes": a[6], "blocks": a[7], "lanes": a[8],
+                "packed_bits": a[9]}
 
     def device_heights(self):
         d = C.c_void_p()

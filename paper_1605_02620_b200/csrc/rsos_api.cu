@@ -489,6 +489,8 @@ extern "C" int rsos_info(rsos_ctx *c, uint64_t *out)
     out[5] = (uint64_t)c->sm_count;
     out[6] = c->smem_bytes;
     out[7] = c->blocks;
+    out[8] = c->p.pk ? c->p.KL : 0;
+    out[9] = c->p.pk ? c->p.FB : 0;
     return RSOS_OK;
 }
 
