@@ -247,7 +247,8 @@ def run_b200(args):
     engine = {"auto": 0, "simple": 1, "warp": 2, "onchip": 3, "thread": 4}[args.engine]
     stream = torch.cuda.Stream()
     heights = torch.empty((R, L, L), dtype=torch.int32, device="cuda")      # device memory only: plumbing
-    g = pkg.Rsos(L, N, R, c["seed"], tile=c["tile"], subsweeps=c["subsweeps"], first_real=rank * R, engine=engine,
+    first_real, _ = workloads.replica_range(rank, world, R)
+    g = pkg.Rsos(L, N, R, c["seed"], tile=c["tile"], subsweeps=c["subsweeps"], first_real=first_real, engine=engine,
                  d_heights=heights.data_ptr(), stream=stream.cuda_stream, lanes=args.lanes)
     info = g.info()
     att_step = workloads.attempts(L, R, mcs)

@@ -34,3 +34,11 @@ def log_spaced_times(t_max, n=64):
 def attempts(L, R, mcs):
     """1 MCS = L*L attempts per realization (reading Q4)."""
     return int(L) * int(L) * int(R) * int(mcs)
+
+
+def replica_range(rank, world, r_per_gpu):
+    """Multi-GPU = replicas only: rank i owns the global realizations
+    [i * r_per_gpu, (i + 1) * r_per_gpu).  Returns (first_real, R) for rsos_init."""
+    if not 0 <= rank < world:
+        raise ValueError("rank %d outside [0, %d)" % (rank, world))
+    return rank * int(r_per_gpu), int(r_per_gpu)
