@@ -63,7 +63,9 @@ def test_argument_errors_need_no_device(lib_path):
     import paper_1605_02620_b200 as m
     for args, kw, code in [((48, 1, 1, 1), {}, -1), ((64, 0, 1, 1), {}, -1), ((64, 1, 0, 1), {}, -1),
                            ((128, 1, 1, 1), dict(tile=24), -1), ((64, 1, 1, 1), dict(engine=m.ENGINE_WARP), -5),
-                           ((256, 1, 1, 1), dict(engine=m.ENGINE_ONCHIP), -5), ((128, 32, 1, 1), dict(engine=m.ENGINE_WARP), -5)]:
+                           ((256, 1, 1, 1), dict(engine=m.ENGINE_ONCHIP), -5), ((128, 32, 1, 1), dict(engine=m.ENGINE_WARP), -5),
+                           ((128, 1, 1, 1), dict(lanes=3), -1), ((128, 8, 1, 1), dict(engine=m.ENGINE_THREAD), -5),
+                           ((256, 1, 1, 1), dict(engine=m.ENGINE_THREAD, tile=128), -5)]:
         with pytest.raises(m.RsosError) as e:
             m.Rsos(*args, **kw)
         assert e.value.code == code, (args, kw)
