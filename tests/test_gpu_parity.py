@@ -287,3 +287,59 @@ def test_error_paths(rsos):
     g.advance(0)
     assert g.t == 0
     g.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# Full-size configurations in the launch configuration bench.py times (engine auto, default lanes),
+# compared on sampled outputs the oracle can compute one by one: realization r is a pure function
+# of (seed, r, ...), so the oracle follows single realizations of the full run (first_real = r).
+# ---------------------------------------------------------------------------------------------
+def _sampled_realizations(rsos, oracle_mod, cfg, N, mcs, sample, want_engine, want_lanes):
+    from paper_1605_02620_b200.utils import workloads
+    c = dict(workloads.CONFIGS[cfg])
+    g = rsos.Rsos(c["L"], N, c["R"], c["seed"], tile=c["tile"], subsweeps=c["subsweeps"])
+    info = g.info()
+    assert info["engine"] == want_engine and info["lanes"] == want_lanes, info
+    g.advance(mcs)
+    gs1, gs2, gacc = g.sums()                               # from the packed lattice, all realizations
+    for r in sample:
+        o = oracle_mod.Oracle(c["L"], N, 1, c["seed"], tile=c["tile"], subsweeps=c["subsweeps"], first_real=r)
+        o.advance(mcs)
+        os1, os2, oacc = o.sums()
+        assert (gs1[r], gs2[r], gacc[r]) == (os1[0], os2[0], oacc[0]), "%s r=%d sums" % (cfg, r)
+        assert np.array_equal(g.heights(r, 1), o.heights()), "%s r=%d heights" % (cfg, r)
+        o.close()
+    # properties that hold for every realization at any size
+    assert (gs1 == gacc).all()                              # sum h = accepted deposits (flat start)
+    h = g.heights(0, 1)[0]
+    for ax in (0, 1):
+        assert np.abs(h - np.roll(h, 1, axis=ax)).max() <= N    # Eq. (6) on every bond, periodic
+    g.close()
+
+
+def test_c2_full_size_sampled_realizations(rsos, oracle_mod):
+    """BASELINE.json configs[1] (L=1024, N=1, R=128): 8192 tiles per pass, THREAD engine, 4 lanes per tile."""
+    _sampled_realizations(rsos, oracle_mod, "C2", 1, 6, [0, 77, 127], "thread", 4)
+
+
+@pytest.mark.parametrize("N", [1, 4])
+def test_c3_full_size_sampled_realizations(rsos, oracle_mod, N):
+    """configs[2] (L=2048, R=64, N in 1..4): 16384 tiles per pass, 1 lane per tile; N=4 uses 4-bit sites."""
+    _sampled_realizations(rsos, oracle_mod, "C3", N, 3, [0, 63], "thread", 1)
+
+
+def test_c4_full_size_whole_surface(rsos, oracle_mod):
+    """configs[3] (L=32768, N=1, R=1, 4 GiB of int32 heights): the whole surface after 2 MCS (2.1e9 attempts),
+    element by element, plus the exact sums taken from the packed lattice."""
+    L = 32768
+    g = rsos.Rsos(L, 1, 1, 1)
+    assert g.info()["engine"] == "thread" and g.info()["lanes"] == 1
+    o = oracle_mod.Oracle(L, 1, 1, 1)
+    g.advance(2)
+    o.advance(2)
+    assert all((a == b).all() for a, b in zip(g.sums(), o.sums()))
+    hg = g.heights()
+    g.close()
+    ho = o.heights()
+    o.close()
+    assert np.array_equal(hg, ho)
