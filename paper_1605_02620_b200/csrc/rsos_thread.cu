@@ -99,32 +99,32 @@ struct Attempt {
     }
 };
 
-// One step: this lane's attempt (slot v).  Returns 1 if the deposit was accepted.
-template <int LGS, int FB, int KL>
-__device__ __forceinline__ uint32_t thread_step(uint32_t base, uint32_t v, uint32_t N, uint32_t rank)
+// Hazard of this lane's attempt against the lower ranks of its group, from the site keys alone
+// (key = dy * 128 + dx).  Equal or adjacent sites have |d| in {0, 1, 128}; sites in one byte of
+// packed sites lie in one row within 3 (2-bit) or 1 (4-bit) columns.  The test |d| <= 3 or
+// |d| == 128 covers both and is conservative: a false alarm only costs a reload.
+template <int KL>
+__device__ __forceinline__ bool group_hazard(uint32_t key, uint32_t rank)
 {
-    constexpr uint32_t FULL = 0xFFFFFFFFu;
-    Attempt<LGS, FB, KL> a;
-    a.prep(base, v);
-    a.load();
-    uint32_t nw;
-    bool ok = a.decide(N, nw);
-    if (KL == 1) {
-        if (ok) a.store(nw);
-        return ok ? 1u : 0u;
-    }
-    // Hazard against the lower ranks of the group, from the site keys alone (key = dy * 128 + dx).
-    // Equal or adjacent sites have |d| in {0, 1, 128}; sites in one byte of packed sites lie in one
-    // row within 3 (2-bit) or 1 (4-bit) columns.  The test |d| <= 3 or |d| == 128 covers both and is
-    // conservative: a false alarm only costs a reload.
     bool hz = false;
 #pragma unroll
     for (int i = 1; i < KL; ++i) {
-        const uint32_t ko = __shfl_up_sync(FULL, a.key, i);
-        const uint32_t d = a.key - ko;
+        const uint32_t ko = __shfl_up_sync(0xFFFFFFFFu, key, i);
+        const uint32_t d = key - ko;
         const bool bad = (d + 3u <= 6u) | (d == 128u) | (d == 0u - 128u);
         hz |= bad & ((uint32_t)i <= rank);
     }
+    return hz;
+}
+
+// Second half of a step (KL > 1), after the loads of `a` were issued: decide on the snapshot,
+// store unless hazardous, then let the hazardous lanes go rank by rank.  Returns 1 if accepted.
+template <int LGS, int FB, int KL>
+__device__ __forceinline__ uint32_t group_finish(Attempt<LGS, FB, KL> &a, bool hz, uint32_t N, uint32_t rank)
+{
+    constexpr uint32_t FULL = 0xFFFFFFFFu;
+    uint32_t nw;
+    bool ok = a.decide(N, nw);
     if (ok & !hz) a.store(nw);
     __syncwarp();
     if (__any_sync(FULL, hz)) {
@@ -196,26 +196,59 @@ __global__ void __launch_bounds__(32) thread_dt_kernel(Params p, uint32_t u, uin
     const uint32_t tile_id = J * T + I;
     const uint32_t N = p.N;
     uint32_t nacc = 0;
+    if (KL == 1) {
 #pragma unroll 1
-    for (uint32_t batch = 0; batch < A / (8u * KL); ++batch) {
-        const uint4 o = philox4x32_10(batch * KL + rank, tile_id, u, rg, p.k0, p.k1);
-        const uint32_t ow[4] = {o.x, o.y, o.z, o.w};
+        for (uint32_t q = 0; q < A / 8u; ++q) {
+            const uint4 o = philox4x32_10(q, tile_id, u, rg, p.k0, p.k1);
+            const uint32_t ow[4] = {o.x, o.y, o.z, o.w};
 #pragma unroll
-        for (uint32_t w = 0; w < 8; ++w) {
-            uint32_t v;
-            if (KL == 1) {
-                v = (ow[w >> 1] >> (16u * (w & 1u))) & 0xFFFFu;
-            } else if (KL == 2) {                         // attempt 2w + rank of the batch: call w >> 2, slot 2(w & 3) + rank
-                const uint32_t x = __shfl_sync(FULL, ow[w & 3u], grp * KL + (w >> 2));
-                v = rank ? x >> 16 : x & 0xFFFFu;
-            } else {                                      // KL == 4: attempt 4w + rank: call w >> 1, slot 4(w & 1) + rank
-                const uint32_t src = grp * KL + (w >> 1);
-                const uint32_t xa = __shfl_sync(FULL, ow[2u * (w & 1u)], src);
-                const uint32_t xb = __shfl_sync(FULL, ow[2u * (w & 1u) + 1u], src);
-                const uint32_t x = (rank & 2u) ? xb : xa;
-                v = (rank & 1u) ? x >> 16 : x & 0xFFFFu;
+            for (uint32_t w = 0; w < 8; ++w) {
+                At a;
+                a.prep(base, (ow[w >> 1] >> (16u * (w & 1u))) & 0xFFFFu);
+                a.load();
+                uint32_t nw;
+                const bool ok = a.decide(N, nw);
+                if (ok) a.store(nw);
+                nacc += ok ? 1u : 0u;
             }
-            nacc += thread_step<LGS, FB, KL>(base, v, N, rank);
+        }
+    } else {
+        // KL lanes per tile.  The slot shuffles, the address arithmetic and the hazard test of step
+        // w + 1 depend on nothing in memory; they are issued right after the loads of step w so that
+        // they fill its latency instead of lengthening the chain load -> decide -> store -> vote.
+        const uint32_t nbatch = A / (8u * KL);
+        uint4 o = philox4x32_10(rank, tile_id, u, rg, p.k0, p.k1);
+        // slot of step w of the batch whose calls are in (o of every rank): attempt KL*w + rank
+        auto slot_of = [&](const uint4 &c, uint32_t w) -> uint32_t {
+            const uint32_t cw[4] = {c.x, c.y, c.z, c.w};
+            if (KL == 2) {                                // call w >> 2, slot 2(w & 3) + rank
+                const uint32_t x = __shfl_sync(FULL, cw[w & 3u], grp * KL + (w >> 2));
+                return rank ? x >> 16 : x & 0xFFFFu;
+            } else {                                      // KL == 4: call w >> 1, slot 4(w & 1) + rank
+                const uint32_t src = grp * KL + (w >> 1);
+                const uint32_t xa = __shfl_sync(FULL, cw[2u * (w & 1u)], src);
+                const uint32_t xb = __shfl_sync(FULL, cw[2u * (w & 1u) + 1u], src);
+                const uint32_t x = (rank & 2u) ? xb : xa;
+                return (rank & 1u) ? x >> 16 : x & 0xFFFFu;
+            }
+        };
+        At cur;
+        cur.prep(base, slot_of(o, 0u));
+        bool hz = group_hazard<KL>(cur.key, rank);
+#pragma unroll 1
+        for (uint32_t batch = 0; batch < nbatch; ++batch) {
+            const uint4 on = philox4x32_10((batch + 1u) * KL + rank, tile_id, u, rg, p.k0, p.k1);   // last one unused
+#pragma unroll
+            for (uint32_t w = 0; w < 8; ++w) {
+                cur.load();
+                At nxt;
+                nxt.prep(base, w < 7u ? slot_of(o, w + 1u) : slot_of(on, 0u));
+                const bool hzn = group_hazard<KL>(nxt.key, rank);
+                nacc += group_finish<LGS, FB, KL>(cur, hz, N, rank);
+                cur = nxt;
+                hz = hzn;
+            }
+            o = on;
         }
     }
     __syncwarp();
