@@ -108,8 +108,8 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
     if (!is_pow2(L) || L < 4 || L > 65536) return fail(RSOS_EINVAL, "L = %u must be a power of two in [4, 65536]", L);
     if (N < 1 || N > 127) return fail(RSOS_EINVAL, "N = %u must be in [1, 127]", N);
     if (R < 1) return fail(RSOS_EINVAL, "R must be >= 1");
-    if (opt.lanes != 0 && opt.lanes != 1 && opt.lanes != 2 && opt.lanes != 4)
-        return fail(RSOS_EINVAL, "opts.lanes = %u must be 0, 1, 2 or 4", opt.lanes);
+    if (opt.lanes != 0 && opt.lanes != 1 && opt.lanes != 2 && opt.lanes != 4 && opt.lanes != 8)
+        return fail(RSOS_EINVAL, "opts.lanes = %u must be 0, 1, 2, 4 or 8", opt.lanes);
     if (opt.engine > RSOS_ENGINE_THREAD) return fail(RSOS_EINVAL, "unknown engine %u", opt.engine);
     uint32_t S = opt.tile ? opt.tile : 64, K = opt.subsweeps ? opt.subsweeps : 1;
     if (!is_pow2(S) || S < 8) return fail(RSOS_EINVAL, "tile = %u must be a power of two >= 8", S);
@@ -187,6 +187,12 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
         int smc = 0;
         INIT_TRY(cudaDeviceGetAttribute(&smc, cudaDevAttrMultiProcessorCount, dev), RSOS_ECUDA);
         p.KL = opt.lanes ? opt.lanes : thread_dt_lanes_per_tile(pass_tiles, smc);
+        while (!opt.lanes && 8ull * p.KL > (uint64_t)S * S / K) p.KL /= 2;              // a batch is 8 * KL attempts
+        if (8ull * p.KL > (uint64_t)S * S / K) {
+            const int rc_ = fail(RSOS_EINVAL, "opts.lanes = %u needs tile^2 / subsweeps >= %u attempts per tile", p.KL, 8 * p.KL);
+            destroy(c);
+            return rc_;
+        }
         const size_t pk_bytes = bytes / 32 * p.FB;                       // FB bits per site
         INIT_TRY(cudaMalloc(&p.pk, pk_bytes), RSOS_ECUDA);
         INIT_TRY(cudaMalloc(&c->d_s1off, (size_t)R * sizeof(long long)), RSOS_ECUDA);

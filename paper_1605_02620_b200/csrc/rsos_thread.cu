@@ -37,7 +37,7 @@ struct TGeom {
 };
 
 // ---------------------------------------------------------------------------------------------
-// KL lanes share one tile (KL = 1, 2 or 4; 32 / KL tiles per warp).  In every step the KL lanes of a
+// KL lanes share one tile (KL = 1, 2, 4 or 8; 32 / KL tiles per warp).  In every step the KL lanes of a
 // group take KL consecutive attempts a0 + rank on the same snapshot of the tile.  A lane whose site
 // is equal or adjacent to the site of a LOWER rank of its group, or shares a byte of packed sites
 // with it, is "hazardous": it waits until the lower ranks have stored and then loads and decides
@@ -127,17 +127,23 @@ __device__ __forceinline__ uint32_t group_finish(Attempt<LGS, FB, KL> &a, bool h
     bool ok = a.decide(N, nw);
     if (ok & !hz) a.store(nw);
     __syncwarp();
-    if (__any_sync(FULL, hz)) {
+    uint32_t todo = __ballot_sync(FULL, hz);
+    if (todo) {
+        // ranks in ascending order; rank rr occupies the lanes rr, rr + KL, ... of the warp
+#pragma unroll 1
+        for (uint32_t rr = 1; rr < (uint32_t)KL && todo; ++rr) {
+            uint32_t lanes_rr = 0;
 #pragma unroll
-        for (int rr = 1; rr < KL; ++rr) {
-            const bool mine = hz & (rank == (uint32_t)rr);
-            if (__any_sync(FULL, mine)) {
-                if (mine) {
+            for (uint32_t g = 0; g < 32u / KL; ++g) lanes_rr |= 1u << (g * KL);
+            lanes_rr <<= rr;
+            if (todo & lanes_rr) {
+                if (hz & (rank == rr)) {
                     a.load();
                     ok = a.decide(N, nw);
                     if (ok) a.store(nw);
                 }
                 __syncwarp();
+                todo &= ~lanes_rr;
             }
         }
     }
@@ -224,11 +230,17 @@ __global__ void __launch_bounds__(32) thread_dt_kernel(Params p, uint32_t u, uin
             if (KL == 2) {                                // call w >> 2, slot 2(w & 3) + rank
                 const uint32_t x = __shfl_sync(FULL, cw[w & 3u], grp * KL + (w >> 2));
                 return rank ? x >> 16 : x & 0xFFFFu;
-            } else {                                      // KL == 4: call w >> 1, slot 4(w & 1) + rank
+            } else if (KL == 4) {                         // call w >> 1, slot 4(w & 1) + rank
                 const uint32_t src = grp * KL + (w >> 1);
                 const uint32_t xa = __shfl_sync(FULL, cw[2u * (w & 1u)], src);
                 const uint32_t xb = __shfl_sync(FULL, cw[2u * (w & 1u) + 1u], src);
                 const uint32_t x = (rank & 2u) ? xb : xa;
+                return (rank & 1u) ? x >> 16 : x & 0xFFFFu;
+            } else {                                      // KL == 8: call w, slot rank
+                const uint32_t src = grp * KL + w;
+                const uint32_t x0 = __shfl_sync(FULL, cw[0], src), x1 = __shfl_sync(FULL, cw[1], src);
+                const uint32_t x2 = __shfl_sync(FULL, cw[2], src), x3 = __shfl_sync(FULL, cw[3], src);
+                const uint32_t x = (rank & 4u) ? ((rank & 2u) ? x3 : x2) : ((rank & 2u) ? x1 : x0);
                 return (rank & 1u) ? x >> 16 : x & 0xFFFFu;
             }
         };
@@ -314,6 +326,7 @@ static cudaError_t thread_dt_k(const Params &p, uint32_t u, uint32_t colour, uin
         case 1: return thread_dt_t<LGS, FB, 1>(p, u, colour, blocks, st, what, out);
         case 2: return thread_dt_t<LGS, FB, 2>(p, u, colour, blocks, st, what, out);
         case 4: return thread_dt_t<LGS, FB, 4>(p, u, colour, blocks, st, what, out);
+        case 8: return thread_dt_t<LGS, FB, 8>(p, u, colour, blocks, st, what, out);
         default: return cudaErrorInvalidValue;
     }
 }

@@ -101,9 +101,11 @@ def test_dt_warp_engine_equals_oracle(rsos, oracle_mod, L, N, R, S, K, mcs, seed
     (64, 1, 2, 8, 2, 5, 8),          # S = 8, A = 32 attempts per tile
     (128, 1, 1, 64, 128, 2, 11),     # A = 32
 ])
-@pytest.mark.parametrize("lanes", [1, 2, 4])
+@pytest.mark.parametrize("lanes", [1, 2, 4, 8])
 def test_dt_thread_engine_equals_oracle(rsos, oracle_mod, L, N, R, S, K, mcs, seed, lanes):
-    """The lane-per-tile engine (2- or 4-bit sites, bank-interleaved shared memory), 1, 2 or 4 lanes per tile."""
+    """The lane-per-tile engine (2- or 4-bit sites, bank-interleaved shared memory), 1, 2, 4 or 8 lanes per tile."""
+    if 8 * lanes > S * S // K:
+        pytest.skip("a batch of 8 * lanes attempts does not fit the tile")
     g = rsos.Rsos(L, N, R, seed, tile=S, subsweeps=K, engine=rsos.ENGINE_THREAD, lanes=lanes)
     o = oracle_mod.Oracle(L, N, R, seed, tile=S, subsweeps=K)
     assert g.info()["mode"] == "DT" and g.info()["engine"] == "thread"
