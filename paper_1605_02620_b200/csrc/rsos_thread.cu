@@ -54,7 +54,7 @@ struct Attempt {
     uint32_t a0, ac;      // shared-memory byte addresses: word of the left neighbour, word of the site
     uint32_t sl, sc;      // bit positions of the left neighbour / the site inside those words
     uint32_t key;         // dy * 128 + dx: sites are equal or adjacent iff keys differ by 0, 1 or 128
-    uint32_t w0, w1, wu, wd;
+    uint32_t w0, w1, wc, wu, wd;
 
     // v: 16-bit slot, dx = v & (S-1), dy = (v >> LGS) & (S-1)   (D:2 step 6)
     __device__ __forceinline__ void prep(uint32_t base, uint32_t v)
@@ -72,21 +72,23 @@ struct Attempt {
     {
         asm volatile("ld.shared.u32 %0, [%1];" : "=r"(w0) : "r"(a0));
         asm volatile("ld.shared.u32 %0, [%1];" : "=r"(w1) : "r"(a0 + WSB));
+        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(wc) : "r"(ac));          // = w0 or w1; saves a select
         asm volatile("ld.shared.u32 %0, [%1];" : "=r"(wu) : "r"(ac - ROWB));
         asm volatile("ld.shared.u32 %0, [%1];" : "=r"(wd) : "r"(ac + ROWB));
     }
     // Eq. (6) test on the loaded words: rejected iff some neighbour sits at h - N, i.e.
-    // (C - nb) mod 2^FB == N (D:3 (i)).  nw = the site's word with field C turned into C + 1 mod 2^FB.
+    // nb == C - N mod 2^FB (D:3 (i)).  nw = the site's word with field C turned into C + 1 mod 2^FB.
     __device__ __forceinline__ bool decide(uint32_t N, uint32_t &nw) const
     {
         constexpr uint32_t M = G::M;
         const uint32_t t3 = __funnelshift_r(w0, w1, sl);           // fields: L, C, R (garbage above)
-        const uint32_t c = t3 >> FB;
-        const uint32_t okL = ((c - t3) ^ N) & M;
-        const uint32_t okR = ((c - (t3 >> (2 * FB))) ^ N) & M;
-        const uint32_t okU = ((c - (wu >> sc)) ^ N) & M;
-        const uint32_t okD = ((c - (wd >> sc)) ^ N) & M;
-        nw = (a0 == ac ? w0 : w1) ^ (((c ^ (c + 1u)) & M) << sc);
+        const uint32_t c = wc >> sc;                               // C in the low FB bits
+        const uint32_t t = c - N;                                  // the blocking neighbour value, mod 2^FB
+        const uint32_t okL = (t3 ^ t) & M;
+        const uint32_t okR = ((t3 >> (2 * FB)) ^ t) & M;
+        const uint32_t okU = ((wu >> sc) ^ t) & M;
+        const uint32_t okD = ((wd >> sc) ^ t) & M;
+        nw = wc ^ (((c ^ (c + 1u)) & M) << sc);
         return (okL != 0u) & (okR != 0u) & (okU != 0u) & (okD != 0u);
     }
     __device__ __forceinline__ void store(uint32_t nw) const
