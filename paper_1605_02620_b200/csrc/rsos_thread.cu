@@ -353,15 +353,14 @@ static cudaError_t thread_dispatch(const Params &p, uint32_t u, uint32_t colour,
 // word wide (so that tiles of one colour never share a packed word), else 4 bits (N <= 7).
 uint32_t thread_dt_field_bits(uint32_t N, uint32_t S) { return (N <= 1u && S >= 16u) ? 2u : 4u; }
 
-// Lanes per tile (D:4): the fewest of 1, 2, 4 that give a colour pass about six warps per SM.  One
-// lane per tile executes the fewest instructions per attempt; more lanes buy resident warps when a
-// pass has few tiles.  Measured on B200 (G attempts/s at 1 / 2 / 4 / 8 lanes): C4, 2048 warps of
-// tiles: 276 / 277 / 253 / -; C3, 512: 233 / 238 / 209 / -; C2, 256: 110 / 142 / 186 / 143.
+// Lanes per tile (D:4): 2 when a colour pass then has about six warps per SM, else 4.  More lanes per
+// tile cost instructions (shuffles, hazard test, votes) and buy resident warps: a tile window is
+// 1.3 KB of shared memory whoever works on it.  Measured on B200 (G attempts/s at 1 / 2 / 4 / 8
+// lanes): C4, 65536 tiles per pass: 284 / 292 / 253 / -; C3, 16384: 233 / 257 / 209 / -;
+// C2, 8192: 110 / 142 / 195 / 143.
 uint32_t thread_dt_lanes_per_tile(uint64_t pass_tiles, int sm_count)
 {
-    for (uint32_t kl = 1; kl < 4; kl *= 2)
-        if (pass_tiles * kl / 32 >= (uint64_t)sm_count * 6) return kl;
-    return 4;
+    return pass_tiles * 2 / 32 >= (uint64_t)sm_count * 6 ? 2u : 4u;
 }
 
 size_t thread_dt_smem(const Params &p)

@@ -335,7 +335,7 @@ def test_c4_full_size_whole_surface(rsos, oracle_mod):
     element by element, plus the exact sums taken from the packed lattice."""
     L = 32768
     g = rsos.Rsos(L, 1, 1, 1)
-    assert g.info()["engine"] == "thread" and g.info()["lanes"] == 1
+    assert g.info()["engine"] == "thread" and g.info()["lanes"] == 2
     o = oracle_mod.Oracle(L, 1, 1, 1)
     g.advance(2)
     o.advance(2)
