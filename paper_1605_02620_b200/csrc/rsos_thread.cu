@@ -53,7 +53,7 @@ struct Attempt {
     static constexpr uint32_t ROWB = G::PW * WSB;         // byte stride between window rows
     uint32_t a0, ac;      // shared-memory byte addresses: word of the left neighbour, word of the site
     uint32_t sl, sc;      // bit positions of the left neighbour / the site inside those words
-    uint32_t key;         // dy * 128 + dx: sites are equal or adjacent iff keys differ by 0, 1 or 128
+    uint32_t key;         // site code dy * S + dx = the low 2 lg S bits of the slot
     uint32_t w0, w1, wc, wu, wd;
 
     // v: 16-bit slot, dx = v & (S-1), dy = (v >> LGS) & (S-1)   (D:2 step 6)
@@ -66,7 +66,7 @@ struct Attempt {
         ac = row + (bc >> 5) * WSB;
         sl = bl & 31u;
         sc = bc & 31u;
-        key = dy * 128u + dx;
+        key = v & (G::S * G::S - 1u);
     }
     __device__ __forceinline__ void load()
     {
@@ -101,20 +101,26 @@ struct Attempt {
     }
 };
 
-// Hazard of this lane's attempt against the lower ranks of its group, from the site keys alone
-// (key = dy * 128 + dx).  Equal or adjacent sites have |d| in {0, 1, 128}; sites in one byte of
-// packed sites lie in one row within 3 (2-bit) or 1 (4-bit) columns.  The test |d| <= 3 or
-// |d| == 128 covers both and is conservative: a false alarm only costs a reload.
-template <int KL>
+// Hazard between two attempts of one step, from their site codes alone (code = dy * S + dx).  Equal
+// or adjacent sites have |d| in {0, 1, S}; sites in one byte of packed sites lie in one row within 3
+// (2-bit) or 1 (4-bit) columns.  The test |d| <= 3 or |d| == S covers both and is conservative (it
+// also fires across a row end): a false alarm only costs a reload.
+template <int LGS>
+__device__ __forceinline__ bool codes_clash(uint32_t a, uint32_t b)
+{
+    const uint32_t d = a - b;
+    return (d + 3u <= 6u) | (d == (1u << LGS)) | (d == 0u - (1u << LGS));
+}
+
+// Hazard of this lane's attempt against the lower ranks of its group (codes fetched by shuffles).
+template <int LGS, int KL>
 __device__ __forceinline__ bool group_hazard(uint32_t key, uint32_t rank)
 {
     bool hz = false;
 #pragma unroll
     for (int i = 1; i < KL; ++i) {
         const uint32_t ko = __shfl_up_sync(0xFFFFFFFFu, key, i);
-        const uint32_t d = key - ko;
-        const bool bad = (d + 3u <= 6u) | (d == 128u) | (d == 0u - 128u);
-        hz |= bad & ((uint32_t)i <= rank);
+        hz |= codes_clash<LGS>(key, ko) & ((uint32_t)i <= rank);
     }
     return hz;
 }
@@ -246,9 +252,47 @@ __global__ void __launch_bounds__(32) thread_dt_kernel(Params p, uint32_t u, uin
                 return (rank & 1u) ? x >> 16 : x & 0xFFFFu;
             }
         };
+        if (KL == 2) {
+            // Two lanes per tile: the pair swaps its two Philox calls once per batch (4 shuffles), so
+            // both lanes hold calls 2b and 2b + 1.  Step w takes word w of the 8: rank 0 the low half
+            // (attempt 2w), rank 1 the high half (attempt 2w + 1) -- each lane sees its partner's slot
+            // in the same register and needs no shuffle for the hazard test.
+            auto swap4 = [&](const uint4 &c) -> uint4 {
+                return make_uint4(__shfl_xor_sync(FULL, c.x, 1), __shfl_xor_sync(FULL, c.y, 1),
+                                  __shfl_xor_sync(FULL, c.z, 1), __shfl_xor_sync(FULL, c.w, 1));
+            };
+            constexpr uint32_t CM = S * S - 1u;
+            auto mine = [&](uint32_t x) -> uint32_t { return rank ? x >> 16 : x & 0xFFFFu; };
+            auto clash = [&](uint32_t x) -> bool { return (rank != 0u) & codes_clash<LGS>((x >> 16) & CM, x & CM); };
+            uint4 po = swap4(o);
+            uint32_t c[9];
+            c[0] = rank ? po.x : o.x; c[1] = rank ? po.y : o.y; c[2] = rank ? po.z : o.z; c[3] = rank ? po.w : o.w;
+            c[4] = rank ? o.x : po.x; c[5] = rank ? o.y : po.y; c[6] = rank ? o.z : po.z; c[7] = rank ? o.w : po.w;
+            At cur;
+            cur.prep(base, mine(c[0]));
+            bool hz = clash(c[0]);
+#pragma unroll 1
+            for (uint32_t batch = 0; batch < nbatch; ++batch) {
+                const uint4 on = philox4x32_10((batch + 1u) * KL + rank, tile_id, u, rg, p.k0, p.k1);   // last one unused
+                const uint4 pon = swap4(on);
+                c[8] = rank ? pon.x : on.x;
+#pragma unroll
+                for (uint32_t w = 0; w < 8; ++w) {
+                    cur.load();
+                    At nxt;
+                    nxt.prep(base, mine(c[w + 1u]));
+                    const bool hzn = clash(c[w + 1u]);
+                    nacc += group_finish<LGS, FB, KL>(cur, hz, N, rank);
+                    cur = nxt;
+                    hz = hzn;
+                }
+                c[0] = c[8]; c[1] = rank ? pon.y : on.y; c[2] = rank ? pon.z : on.z; c[3] = rank ? pon.w : on.w;
+                c[4] = rank ? on.x : pon.x; c[5] = rank ? on.y : pon.y; c[6] = rank ? on.z : pon.z; c[7] = rank ? on.w : pon.w;
+            }
+        } else {
         At cur;
         cur.prep(base, slot_of(o, 0u));
-        bool hz = group_hazard<KL>(cur.key, rank);
+        bool hz = group_hazard<LGS, KL>(cur.key, rank);
 #pragma unroll 1
         for (uint32_t batch = 0; batch < nbatch; ++batch) {
             const uint4 on = philox4x32_10((batch + 1u) * KL + rank, tile_id, u, rg, p.k0, p.k1);   // last one unused
@@ -257,12 +301,13 @@ __global__ void __launch_bounds__(32) thread_dt_kernel(Params p, uint32_t u, uin
                 cur.load();
                 At nxt;
                 nxt.prep(base, w < 7u ? slot_of(o, w + 1u) : slot_of(on, 0u));
-                const bool hzn = group_hazard<KL>(nxt.key, rank);
+                const bool hzn = group_hazard<LGS, KL>(nxt.key, rank);
                 nacc += group_finish<LGS, FB, KL>(cur, hz, N, rank);
                 cur = nxt;
                 hz = hzn;
             }
             o = on;
+        }
         }
     }
     __syncwarp();
