@@ -108,8 +108,8 @@ struct Attempt {
 template <int LGS>
 __device__ __forceinline__ bool codes_clash(uint32_t a, uint32_t b)
 {
-    const uint32_t d = a - b;
-    return (d + 3u <= 6u) | (d == (1u << LGS)) | (d == 0u - (1u << LGS));
+    const uint32_t d = (uint32_t)abs((int32_t)(a - b));
+    return (d <= 3u) | (d == (1u << LGS));
 }
 
 // Hazard of this lane's attempt against the lower ranks of its group (codes fetched by shuffles).
