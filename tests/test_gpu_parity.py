@@ -345,3 +345,59 @@ def test_c4_full_size_whole_surface(rsos, oracle_mod):
     ho = o.heights()
     o.close()
     assert np.array_equal(hg, ho)
+
+
+# ---------------------------------------------------------------------------------------------
+# Snapshot induction at late times (rough surfaces), full size: the GPU state at time t is handed to
+# the oracle (t enters the Philox counter, so (heights, t) is the whole state), both advance, and
+# the results must be equal.  Together with the exact prefixes above this covers the whole run by
+# induction on the sampled steps.
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("t0", [300, 1500])
+def test_c2_full_size_snapshot_induction(rsos, oracle_mod, t0):
+    """C2 in full (128 realizations, bench launch configuration): realizations 3 and 126 at time t0 go to the
+    oracle, the full GPU run and the oracle both advance 2 MCS, and those realizations must be equal."""
+    from paper_1605_02620_b200.utils import workloads
+    c = dict(workloads.CONFIGS["C2"])
+    g = rsos.Rsos(c["L"], c["N"], c["R"], c["seed"], tile=c["tile"], subsweeps=c["subsweeps"])
+    assert g.info()["engine"] == "thread"
+    g.advance(t0)
+    acc = g.sums()[2]
+    oracles = {}
+    for r in (3, 126):
+        h0 = g.heights(r, 1)
+        for ax in (0, 1):
+            assert np.abs(h0[0] - np.roll(h0[0], 1, axis=ax)).max() <= c["N"]
+        assert h0.max() - h0.min() > 8                      # a rough surface, not the flat start
+        o = oracle_mod.Oracle(c["L"], c["N"], 1, c["seed"], tile=c["tile"], subsweeps=c["subsweeps"], first_real=r)
+        o.set_state(h0, t0, acc[r:r + 1])
+        o.advance(2)
+        oracles[r] = o
+    g.advance(2)
+    gs1, gs2, gacc = g.sums()
+    for r, o in oracles.items():
+        os1, os2, oacc = o.sums()
+        assert (gs1[r], gs2[r], gacc[r]) == (os1[0], os2[0], oacc[0]), "r=%d sums" % r
+        assert np.array_equal(g.heights(r, 1), o.heights()), "r=%d heights" % r
+        o.close()
+    g.close()
+
+
+def test_c4_full_size_snapshot_induction(rsos, oracle_mod):
+    """C4: the whole 2^30-site surface at t = 40 goes to the oracle; both advance 1 MCS; all heights equal."""
+    L = 32768
+    g = rsos.Rsos(L, 1, 1, 1)
+    g.advance(40)
+    h0 = g.heights()
+    acc = g.sums()[2]
+    o = oracle_mod.Oracle(L, 1, 1, 1)
+    o.set_state(h0, 40, acc)
+    del h0
+    g.advance(1)
+    o.advance(1)
+    assert all((a == b).all() for a, b in zip(g.sums(), o.sums()))
+    hg = g.heights()
+    g.close()
+    ho = o.heights()
+    o.close()
+    assert np.array_equal(hg, ho)
