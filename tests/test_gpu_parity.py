@@ -401,3 +401,18 @@ def test_c4_full_size_snapshot_induction(rsos, oracle_mod):
     ho = o.heights()
     o.close()
     assert np.array_equal(hg, ho)
+
+
+def test_dd_consistency_table_on_gpu(rsos):
+    """SURVEY 8(f) NEXT-1 / DESIGN.md section 12: the tile side sets the bias of the decomposed schedule against
+    serial RS ("domain size ... noise amplitude").  Deterministic (fixed seeds); values recorded in DESIGN.md."""
+    from paper_1605_02620_b200 import dd_consistency
+    rows = dd_consistency.table(L=128, N=1, R=4096, seed=1, times=(1, 10, 100))
+    dev = {name: d for name, _, _, d in rows if d is not None}
+    bias_t1 = [abs(dev["DT(%d,1)" % S][0][0]) for S in (8, 16, 32, 64)]
+    assert bias_t1 == sorted(bias_t1, reverse=True) and bias_t1[0] > 0.03 > 0.006 > bias_t1[3]
+    for i in range(3):                                      # the fidelity setting agrees with serial dynamics
+        dw, sdw, dh, sdh = dev["DT(64,4)"][i]
+        assert abs(dw) < 4 * sdw and abs(dh) < 5e-4
+    dw, sdw, _, _ = dev["DT(64,1)"][2]                      # the default: unresolvable from t ~ 100 on
+    assert abs(dw) < 3 * sdw
