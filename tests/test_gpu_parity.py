@@ -416,3 +416,19 @@ def test_dd_consistency_table_on_gpu(rsos):
         assert abs(dw) < 4 * sdw and abs(dh) < 5e-4
     dw, sdw, _, _ = dev["DT(64,1)"][2]                      # the default: unresolvable from t ~ 100 on
     assert abs(dw) < 3 * sdw
+
+
+def test_growth_exponent_sanity_c2(rsos):
+    """Loose physics pin P10 (not parity): on C2 the slope of ln<W^2> vs ln t over t in [100, 3200] is 2 beta with
+    beta = 0.241(1) in the paper.  Measured on the B200: 0.4754."""
+    from paper_1605_02620_b200.utils import workloads
+    c = dict(workloads.CONFIGS["C2"])
+    g = rsos.Rsos(c["L"], c["N"], c["R"], c["seed"], tile=c["tile"], subsweeps=c["subsweeps"])
+    ts, t, w = [100, 200, 400, 800, 1600, 3200], 0, []
+    for tt in ts:
+        g.advance(tt - t)
+        t = tt
+        w.append(g.width()[0].mean())
+    g.close()
+    slope = np.polyfit(np.log(ts), np.log(w), 1)[0]
+    assert 0.45 < slope < 0.50, slope
