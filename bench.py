@@ -85,14 +85,17 @@ def l2_note(c, info):
 
 
 def traffic_note(workload_name, info):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full summary (profiles/), or None."""
-    path = os.path.join(ROOT, "profiles", "traffic.json")
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full summary (profiles/traffic.csv), or None."""
+    key = "%s/%s/lanes%d" % (workload_name, info["engine"], info.get("lanes", 0))
     try:
-        with open(path) as f:
-            t = json.load(f)
-        return t.get("%s/%s/lanes%d" % (workload_name, info["engine"], info.get("lanes", 0)))
+        with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
+            for line in f:
+                parts = line.strip().split(",")
+                if len(parts) == 2 and parts[0] == key:
+                    return float(parts[1])
     except (OSError, ValueError):
-        return None
+        pass
+    return None
 
 
 def config_dict(args, c, n_gpus, info=None):
