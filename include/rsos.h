@@ -80,8 +80,9 @@ typedef struct rsos_opts {
                           /* rsos_moments, rsos_set_state and rsos_device_heights.                */
     void    *stream;      /* cudaStream_t to enqueue on; NULL = the legacy default stream         */
     int32_t  device;      /* CUDA device ordinal + 1; 0 = the current device                      */
-    uint32_t lanes;       /* THREAD engine: lanes that share one tile, 1, 2 or 4; 0 = chosen from the     */
-                          /* number of tiles per colour pass (D:4).  Does not change the result.          */
+    uint32_t lanes;       /* THREAD engine: lanes that share one tile, 1, 2, 4 or 8 (8 * lanes must not   */
+                          /* exceed tile^2 / subsweeps); 0 = chosen from the number of tiles per colour   */
+                          /* pass (D:4).  Does not change the result.                                     */
 } rsos_opts;
 
 /*
