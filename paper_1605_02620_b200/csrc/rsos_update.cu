@@ -267,7 +267,7 @@ __global__ void __launch_bounds__(WARP_DT_WARPS * 32) warp_dt_kernel(Params p, u
     // ---- stage: rows y0-1 .. y0+S, columns xa .. xa+S+7, low 6 bits of each height ----------
     {
         uint16_t *sm16 = reinterpret_cast<uint16_t *>(sm);
-#pragma unroll 4
+#pragma unroll 12
         for (uint32_t it = lane; it < NROW * NCH; it += 32u) {
             const uint32_t yr = it / NCH, c = it - yr * NCH;
             const uint32_t Y = offy - 1u + yr;
@@ -288,17 +288,33 @@ __global__ void __launch_bounds__(WARP_DT_WARPS * 32) warp_dt_kernel(Params p, u
 
     // ---- write back: int32 heights rebuilt column by column from the frozen halo row ----------
     // h(x, y) = h(x, y-1) + sext6(b(x, y) - b(x, y-1)): adjacent heights differ by <= N <= 31.
-#pragma unroll 1
-    for (uint32_t cx = lane; cx < S; cx += 32u) {
-        const uint32_t X = offx + cx, gx = (x0 + cx) & Lm;
-        int32_t hv = h[(size_t)((y0 - 1u) & Lm) * L + gx];
-        uint32_t bprev = sm_height<LGS, false>(sm, X, offy - 1u);
-#pragma unroll 8
+    // All column groups of a lane advance together so that their halo loads and chains overlap.
+    {
+        constexpr uint32_t NG = (S + 31u) / 32u;
+        int32_t hv[NG];
+        uint32_t bprev[NG];
+#pragma unroll
+        for (uint32_t g = 0; g < NG; ++g) {
+            const uint32_t cx = lane + 32u * g;
+            hv[g] = 0; bprev[g] = 0;
+            if (cx < S) {
+                hv[g] = h[(size_t)((y0 - 1u) & Lm) * L + ((x0 + cx) & Lm)];
+                bprev[g] = sm_height<LGS, false>(sm, offx + cx, offy - 1u);
+            }
+        }
+#pragma unroll 4
         for (uint32_t dy = 0; dy < S; ++dy) {
-            const uint32_t b = sm_height<LGS, false>(sm, X, offy + dy);
-            hv += sext6(b - bprev);
-            bprev = b;
-            h[(size_t)((y0 + dy) & Lm) * L + gx] = hv;
+            int32_t *grow = h + (size_t)((y0 + dy) & Lm) * L;
+#pragma unroll
+            for (uint32_t g = 0; g < NG; ++g) {
+                const uint32_t cx = lane + 32u * g;
+                if (cx < S) {
+                    const uint32_t b = sm_height<LGS, false>(sm, offx + cx, offy + dy);
+                    hv[g] += sext6(b - bprev[g]);
+                    bprev[g] = b;
+                    grow[(x0 + cx) & Lm] = hv[g];
+                }
+            }
         }
     }
     const uint32_t tot = __reduce_add_sync(0xFFFFFFFFu, my_acc);
