@@ -9,7 +9,7 @@ namespace rsos {
 
 struct Params;
 
-constexpr int WARP_DT_WARPS = 8;     // warps (= tiles) per block of the DT warp engine
+constexpr int WARP_DT_WARPS = 1;     // warps (= tiles) per block of the DT warp engine (1: even spread over SMs)
 constexpr int WARP_RS_WARPS = 4;     // warps (= realizations) per block of the on-chip RS engine
 
 enum : uint32_t { ENGINE_AUTO = 0, ENGINE_SIMPLE = 1, ENGINE_WARP = 2, ENGINE_ONCHIP = 3, ENGINE_THREAD = 4 };
