@@ -186,7 +186,7 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
         p.FB = thread_dt_field_bits(N, S);
         int smc = 0;
         INIT_TRY(cudaDeviceGetAttribute(&smc, cudaDevAttrMultiProcessorCount, dev), RSOS_ECUDA);
-        p.KL = opt.lanes ? opt.lanes : thread_dt_lanes_per_tile(pass_tiles, smc);
+        p.KL = opt.lanes ? opt.lanes : thread_dt_lanes_per_tile(pass_tiles, smc, p.FB);
         while (!opt.lanes && 8ull * p.KL > (uint64_t)S * S / K) p.KL /= 2;              // a batch is 8 * KL attempts
         if (8ull * p.KL > (uint64_t)S * S / K) {
             const int rc_ = fail(RSOS_EINVAL, "opts.lanes = %u needs tile^2 / subsweeps >= %u attempts per tile", p.KL, 8 * p.KL);

@@ -25,7 +25,7 @@ cudaError_t launch_philox(const uint32_t *d_ctr, const uint32_t *d_key, uint32_t
 
 // rsos_thread.cu (lane-per-tile DT engine on the packed lattice)
 uint32_t thread_dt_field_bits(uint32_t N, uint32_t S);
-uint32_t thread_dt_lanes_per_tile(uint64_t pass_tiles, int sm_count);
+uint32_t thread_dt_lanes_per_tile(uint64_t pass_tiles, int sm_count, uint32_t field_bits);
 size_t thread_dt_smem(const Params &p);
 cudaError_t thread_dt_configure(const Params &p);
 uint32_t thread_dt_blocks(const Params &p);

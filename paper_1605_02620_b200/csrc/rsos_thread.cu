@@ -403,8 +403,11 @@ uint32_t thread_dt_field_bits(uint32_t N, uint32_t S) { return (N <= 1u && S >= 
 // 1.3 KB of shared memory whoever works on it.  Measured on B200 (G attempts/s at 1 / 2 / 4 / 8
 // lanes): C4, 65536 tiles per pass: 284 / 292 / 253 / -; C3, 16384: 233 / 257 / 209 / -;
 // C2, 8192: 110 / 142 / 195 / 143.
-uint32_t thread_dt_lanes_per_tile(uint64_t pass_tiles, int sm_count)
+// With 4-bit sites a window is twice as large (half the resident warps): 4 lanes (C3 at N = 2..4:
+// 112 / 156 / 174 G attempts/s at 1 / 2 / 4 lanes).
+uint32_t thread_dt_lanes_per_tile(uint64_t pass_tiles, int sm_count, uint32_t field_bits)
 {
+    if (field_bits > 2) return 4u;
     return pass_tiles * 2 / 32 >= (uint64_t)sm_count * 6 ? 2u : 4u;
 }
 

@@ -327,7 +327,7 @@ def test_c2_full_size_sampled_realizations(rsos, oracle_mod):
 @pytest.mark.parametrize("N", [1, 4])
 def test_c3_full_size_sampled_realizations(rsos, oracle_mod, N):
     """configs[2] (L=2048, R=64, N in 1..4): 16384 tiles per pass, 2 lanes per tile; N=4 uses 4-bit sites."""
-    _sampled_realizations(rsos, oracle_mod, "C3", N, 3, [0, 63], "thread", 2)
+    _sampled_realizations(rsos, oracle_mod, "C3", N, 3, [0, 63], "thread", 2 if N == 1 else 4)
 
 
 def test_c4_full_size_whole_surface(rsos, oracle_mod):
