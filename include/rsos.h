@@ -174,6 +174,15 @@ int rsos_device_heights(rsos_ctx *ctx, int32_t **d);
  */
 int rsos_kernel_time(rsos_ctx *ctx, int enable, double *ms_total, uint64_t *n_launches);
 
+/*
+ * rsos_plan -- what rsos_init would choose for (L, N, R, opts) on a device with sm_count SMs
+ * (<= 0: 148, a B200): pure host logic, needs no CUDA device.  out (host, 8 uint64): out[0] = mode
+ * (0 RS, 1 DT), out[1] = engine, out[2] = S, out[3] = K, out[4] = active tiles per colour pass
+ * (0 in RS mode), out[5] = THREAD engine lanes per tile (else 0), out[6] = bits per site of the
+ * packed lattice (else 0), out[7] = kernel launches per MCS.  Same argument errors as rsos_init.
+ */
+int rsos_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts *opts, int sm_count, uint64_t *out);
+
 /* rsos_free -- release the context and everything the library allocated (not d_heights). */
 void rsos_free(rsos_ctx *ctx);
 

@@ -19,7 +19,7 @@ RSOS_OK, RSOS_EINVAL, RSOS_ERANGE, RSOS_ENOMEM, RSOS_ECUDA, RSOS_EUNSUP = 0, -1,
 # every symbol include/rsos.h declares (tests check the .so exports exactly these)
 SYMBOLS = ("rsos_init", "rsos_advance", "rsos_sums", "rsos_width", "rsos_moments", "rsos_get_heights",
            "rsos_set_state", "rsos_time", "rsos_info", "rsos_device_heights", "rsos_kernel_time",
-           "rsos_free", "rsos_last_error", "rsos_philox")
+           "rsos_free", "rsos_last_error", "rsos_philox", "rsos_plan")
 
 
 class RsosOpts(C.Structure):
@@ -69,6 +69,15 @@ def load():
 def _check(rc):
     if rc != 0:
         raise RsosError(rc, load().rsos_last_error().decode())
+
+
+def plan(L, N, R, tile=0, subsweeps=0, engine=ENGINE_AUTO, lanes=0, sm_count=0):
+    """rsos_plan: what rsos_init would choose for these arguments (host only, no device needed)."""
+    o = RsosOpts(int(tile), int(subsweeps), 0, int(engine), None, None, 0, int(lanes))
+    a = (C.c_uint64 * 8)()
+    _check(load().rsos_plan(int(L), int(N), int(R), C.byref(o), int(sm_count), a))
+    return {"mode": "DT" if a[0] else "RS", "engine": ENGINE_NAMES[a[1]], "S": a[2], "K": a[3], "pass_tiles": a[4],
+            "lanes": a[5], "packed_bits": a[6], "launches_per_mcs": a[7]}
 
 
 def philox(ctr, key):

@@ -98,13 +98,16 @@ static void destroy(rsos_ctx *c)
     delete c;
 }
 
-extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uint64_t seed, const rsos_opts *o)
+// Host-only planning: argument checks, mode, engine selection, lanes and packed-site width.
+// Shared by rsos_init and rsos_plan; needs no device.
+struct Plan {
+    bool mode_dt;
+    uint32_t engine, S, K, lanes, field_bits;
+    uint64_t pass_tiles;
+};
+
+static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, int sm_count, Plan *pl)
 {
-    if (!out) return fail(RSOS_EINVAL, "ctx is NULL");
-    *out = nullptr;
-    rsos_opts opt;
-    memset(&opt, 0, sizeof opt);
-    if (o) opt = *o;
     if (!is_pow2(L) || L < 4 || L > 65536) return fail(RSOS_EINVAL, "L = %u must be a power of two in [4, 65536]", L);
     if (N < 1 || N > 127) return fail(RSOS_EINVAL, "N = %u must be in [1, 127]", N);
     if (R < 1) return fail(RSOS_EINVAL, "R must be >= 1");
@@ -141,12 +144,60 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
         return fail(RSOS_EUNSUP, "engine THREAD needs DT mode (2*tile <= L), tile <= 64 and N <= 7");
     if (engine == RSOS_ENGINE_ONCHIP && !onchip_ok)
         return fail(RSOS_EUNSUP, "engine ONCHIP needs RS mode (2*tile > L), L <= 128 and N <= 31");
+    pl->mode_dt = mode_dt; pl->engine = engine; pl->S = S; pl->K = K; pl->pass_tiles = pass_tiles;
+    pl->lanes = 0; pl->field_bits = 0;
+    if (engine == RSOS_ENGINE_THREAD) {
+        pl->field_bits = thread_dt_field_bits(N, S);
+        uint32_t kl = opt.lanes ? opt.lanes : thread_dt_lanes_per_tile(pass_tiles, sm_count, pl->field_bits);
+        while (!opt.lanes && 8ull * kl > (uint64_t)S * S / K) kl /= 2;                       // a batch is 8 * lanes attempts
+        if (8ull * kl > (uint64_t)S * S / K)
+            return fail(RSOS_EINVAL, "opts.lanes = %u needs tile^2 / subsweeps >= %u attempts per tile", kl, 8 * kl);
+        pl->lanes = kl;
+    }
+    return RSOS_OK;
+}
 
+extern "C" int rsos_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts *o, int sm_count, uint64_t *out)
+{
+    if (!out) return fail(RSOS_EINVAL, "out is NULL");
+    rsos_opts opt;
+    memset(&opt, 0, sizeof opt);
+    if (o) opt = *o;
+    Plan pl;
+    const int rc = make_plan(L, N, R, opt, sm_count > 0 ? sm_count : 148, &pl);
+    if (rc) return rc;
+    out[0] = pl.mode_dt ? 1 : 0; out[1] = pl.engine; out[2] = pl.S; out[3] = pl.K;
+    out[4] = pl.pass_tiles; out[5] = pl.lanes; out[6] = pl.field_bits;
+    out[7] = pl.mode_dt ? (uint64_t)4 * pl.K : 1;                                             // launches per MCS
+    return RSOS_OK;
+}
+
+extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uint64_t seed, const rsos_opts *o)
+{
+    if (!out) return fail(RSOS_EINVAL, "ctx is NULL");
+    *out = nullptr;
+    rsos_opts opt;
+    memset(&opt, 0, sizeof opt);
+    if (o) opt = *o;
+
+    Plan pl;
+    {   // argument errors are reported before any device is touched
+        const int rc0 = make_plan(L, N, R, opt, 148, &pl);
+        if (rc0) return rc0;
+    }
     int dev = 0;
     if (opt.device > 0) dev = opt.device - 1;
     else CUDA_TRY(cudaGetDevice(&dev));
     DeviceGuard guard(dev);
     if (!guard.ok) return fail(RSOS_ECUDA, "cannot select CUDA device %d", dev);
+    {
+        int smc = 0;
+        CUDA_TRY(cudaDeviceGetAttribute(&smc, cudaDevAttrMultiProcessorCount, dev));
+        const int rc0 = make_plan(L, N, R, opt, smc, &pl);
+        if (rc0) return rc0;
+    }
+    const bool mode_dt = pl.mode_dt;
+    const uint32_t engine = pl.engine, S = pl.S, K = pl.K;
 
     rsos_ctx *c = new (std::nothrow) rsos_ctx();
     if (!c) return fail(RSOS_ENOMEM, "out of host memory");
@@ -183,16 +234,8 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
     INIT_TRY(cudaMalloc(&c->d_base, (size_t)R * sizeof(long long)), RSOS_ECUDA);
     c->h_valid = c->pk_valid = true;
     if (engine == RSOS_ENGINE_THREAD) {
-        p.FB = thread_dt_field_bits(N, S);
-        int smc = 0;
-        INIT_TRY(cudaDeviceGetAttribute(&smc, cudaDevAttrMultiProcessorCount, dev), RSOS_ECUDA);
-        p.KL = opt.lanes ? opt.lanes : thread_dt_lanes_per_tile(pass_tiles, smc, p.FB);
-        while (!opt.lanes && 8ull * p.KL > (uint64_t)S * S / K) p.KL /= 2;              // a batch is 8 * KL attempts
-        if (8ull * p.KL > (uint64_t)S * S / K) {
-            const int rc_ = fail(RSOS_EINVAL, "opts.lanes = %u needs tile^2 / subsweeps >= %u attempts per tile", p.KL, 8 * p.KL);
-            destroy(c);
-            return rc_;
-        }
+        p.FB = pl.field_bits;
+        p.KL = pl.lanes;
         const size_t pk_bytes = bytes / 32 * p.FB;                       // FB bits per site
         INIT_TRY(cudaMalloc(&p.pk, pk_bytes), RSOS_ECUDA);
         INIT_TRY(cudaMalloc(&c->d_s1off, (size_t)R * sizeof(long long)), RSOS_ECUDA);

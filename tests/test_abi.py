@@ -82,3 +82,32 @@ def test_product_never_touches_the_oracle():
         if f.endswith((".py", ".c")):
             text = open(os.path.join(ROOT, "oracle", f)).read()
             assert not re.search(r"^\s*(from|import)\s+paper_1605_02620_b200|#include\s+\".*csrc", text, flags=re.M), f
+
+
+def test_plan_picks_engines_lanes_and_site_width(lib_path):
+    """rsos_plan: the host-side selection logic of rsos_init, no device needed."""
+    import paper_1605_02620_b200 as m
+    from paper_1605_02620_b200.utils import workloads as w
+    c = w.CONFIGS
+    p = m.plan(c["C1"]["L"], 1, c["C1"]["R"])
+    assert (p["mode"], p["engine"], p["S"], p["K"], p["launches_per_mcs"]) == ("RS", "onchip", 32, 1, 1)
+    p = m.plan(c["C2"]["L"], 1, c["C2"]["R"])
+    assert (p["mode"], p["engine"], p["pass_tiles"], p["lanes"], p["packed_bits"]) == ("DT", "thread", 8192, 4, 2)
+    p = m.plan(c["C3"]["L"], 1, c["C3"]["R"])
+    assert (p["engine"], p["pass_tiles"], p["lanes"], p["packed_bits"]) == ("thread", 16384, 2, 2)
+    p = m.plan(c["C3"]["L"], 4, c["C3"]["R"])
+    assert (p["engine"], p["lanes"], p["packed_bits"]) == ("thread", 4, 4)         # 4-bit sites for N = 2..7
+    p = m.plan(c["C4"]["L"], 1, 1)
+    assert (p["engine"], p["pass_tiles"], p["lanes"], p["launches_per_mcs"]) == ("thread", 65536, 2, 4)
+    p = m.plan(128, 1, w.c5_realizations(128), tile=64, subsweeps=4)                  # C5 at L = 128: few tiles per pass
+    assert (p["engine"], p["pass_tiles"], p["launches_per_mcs"]) == ("warp", 1024, 16)
+    assert m.plan(64, 1, 4096)["engine"] == "onchip" and m.plan(512, 1, 2, tile=512)["engine"] == "simple"
+    assert m.plan(256, 8, 4096)["engine"] == "warp" and m.plan(256, 40, 4096)["engine"] == "simple"
+    assert m.plan(1024, 1, 128, tile=8)["packed_bits"] == 4                          # 8 < 16 sites per 2-bit word
+    assert m.plan(1024, 1, 128, subsweeps=128)["lanes"] == 4                         # 32 attempts per tile: 8 * 4 fits
+    assert m.plan(1024, 1, 128, subsweeps=128, engine=m.ENGINE_THREAD, lanes=2)["lanes"] == 2
+    with pytest.raises(m.RsosError) as e:
+        m.plan(1024, 1, 128, subsweeps=128, engine=m.ENGINE_THREAD, lanes=8)         # a batch of 64 attempts does not fit
+    assert e.value.code == -1
+    # fewer SMs: the same pass reaches six warps per SM with fewer lanes
+    assert m.plan(c["C2"]["L"], 1, c["C2"]["R"], sm_count=16)["lanes"] == 2
