@@ -257,8 +257,10 @@ def test_invariants_on_device_result(rsos, oracle_mod):
     g.close()
 
 
-def test_moments_exact(rsos):
-    g = rsos.Rsos(256, 3, 2, 5)
+@pytest.mark.parametrize("engine", ["auto", "thread"])
+def test_moments_exact(rsos, engine):
+    """rsos_moments right after rsos_advance: with the THREAD engine it has to rebuild the int32 heights first."""
+    g = rsos.Rsos(256, 3, 2, 5, engine=rsos.ENGINE_THREAD if engine == "thread" else rsos.ENGINE_AUTO)
     g.advance(6)
     base, M = g.moments()
     h = g.heights()
