@@ -82,13 +82,23 @@ struct Attempt {
     {
         constexpr uint32_t M = G::M;
         const uint32_t t3 = __funnelshift_r(w0, w1, sl);           // fields: L, C, R (garbage above)
-        const uint32_t c = wc >> sc;                               // C in the low FB bits
-        const uint32_t t = c - N;                                  // the blocking neighbour value, mod 2^FB
-        const uint32_t okL = (t3 ^ t) & M;
-        const uint32_t okR = ((t3 >> (2 * FB)) ^ t) & M;
-        const uint32_t okU = ((wu >> sc) ^ t) & M;
-        const uint32_t okD = ((wd >> sc) ^ t) & M;
-        nw = wc ^ (((c ^ (c + 1u)) & M) << sc);
+        // Everything is compared in the TOP FB bits of a register: a field is moved there by a multiply
+        // with 2^(32 - FB - position) (IMAD: the fma pipe) instead of a shift (the alu pipe, which is
+        // what this loop saturates first -- D:6).
+        constexpr uint32_t TOP = M << (32 - FB), ONE = 1u << (32 - FB);
+        const uint32_t m = ONE >> sc;                              // 2^(32 - FB - sc)
+        auto mul = [](uint32_t a, uint32_t b) -> uint32_t {         // a real multiply: ptxas would turn a * 2^k into a shift
+            uint32_t r;
+            asm("mul.lo.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));
+            return r;
+        };
+        const uint32_t ct = mul(wc, m);                            // C on top
+        const uint32_t tt = ct - N * ONE;                          // the blocking neighbour value C - N on top
+        const uint32_t okL = ((t3 * ONE) ^ tt) & TOP;
+        const uint32_t okR = ((t3 * (ONE >> (2 * FB))) ^ tt) & TOP;
+        const uint32_t okU = (mul(wu, m) ^ tt) & TOP;
+        const uint32_t okD = (mul(wd, m) ^ tt) & TOP;
+        nw = wc ^ (((ct ^ (ct + ONE)) & TOP) >> (32 - FB - sc));   // field + 1 mod 2^FB
         return (okL != 0u) & (okR != 0u) & (okU != 0u) & (okD != 0u);
     }
     __device__ __forceinline__ void store(uint32_t nw) const
