@@ -140,7 +140,10 @@ int rsos_get_heights(rsos_ctx *ctx, uint32_t r0, uint32_t nr, int32_t *host_out)
  * rsos_set_state -- overwrite realizations r0 .. r0+nr-1 from host_in (same layout), set the sweep
  * counter t (applies to all realizations) and, if accepted != NULL, their accepted counters
  * (host, nr int64).  For snapshot restarts: t enters the Philox counter, so (heights, t) is the
- * whole state.  The caller guarantees Eq. (6) holds in host_in.  Synchronises the stream.
+ * whole state.  Synchronises the stream.  Every engine relies on Eq. (6), so the written surfaces
+ * are checked on the device: if some bond has |dh| > N the call returns RSOS_EINVAL -- the one
+ * failure WITH an effect: the realizations hold host_in and t is set, and a valid state must be
+ * set before the next rsos_advance.
  */
 int rsos_set_state(rsos_ctx *ctx, uint32_t r0, uint32_t nr, const int32_t *host_in,
                    uint64_t t, const int64_t *accepted);

@@ -515,8 +515,16 @@ extern "C" int rsos_set_state(rsos_ctx *c, uint32_t r0, uint32_t nr, const int32
     if (nr) CUDA_TRY(cudaMemcpyAsync(c->p.h + r0 * per, host_in, nr * per * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
     if (nr && accepted)
         CUDA_TRY(cudaMemcpyAsync(c->p.accepted + r0, accepted, nr * sizeof(int64_t), cudaMemcpyHostToDevice, c->stream));
+    if (nr) {                                              // every engine relies on Eq. (6): check what was written
+        CUDA_TRY(launch_violations(c->p.h + r0 * per, c->p.L, c->p.lgL, nr, c->p.N, c->d_red, c->stream));
+        ++c->launches;
+        CUDA_TRY(cudaMemcpyAsync(c->h_red, c->d_red, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+    }
     CUDA_TRY(cudaStreamSynchronize(c->stream));
     c->t = t;
+    if (nr && c->h_red[0])
+        return fail(RSOS_EINVAL, "host_in violates Eq. (6) on %llu bonds (|dh| > N = %u); set a valid state before advancing",
+                    c->h_red[0], c->p.N);
     return RSOS_OK;
 }
 

@@ -137,4 +137,38 @@ cudaError_t launch_moments(const int32_t *h, uint32_t L, uint32_t R, const long 
     return cudaSuccess;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Eq. (6) check of nr surfaces: counts the bonds (x, x+1) and (y, y+1), periodic, with
+// |dh| > N into *d_bad.  Used by rsos_set_state: every engine relies on the invariant.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(RED_THREADS) violations_kernel(const int32_t *__restrict__ h, uint32_t L, uint32_t lgL,
+                                                                 int32_t N, unsigned long long *d_bad)
+{
+    const int32_t *s = h + ((size_t)blockIdx.y << (2 * lgL));
+    const uint32_t Lm = L - 1;
+    unsigned int bad = 0;
+    for (uint64_t i = (uint64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < ((uint64_t)1 << (2 * lgL)); i += (uint64_t)gridDim.x * RED_THREADS) {
+        const uint32_t x = (uint32_t)i & Lm, y = (uint32_t)(i >> lgL);
+        const int32_t c = s[i];
+        const int32_t r = s[((size_t)y << lgL) + ((x + 1) & Lm)], d = s[((size_t)((y + 1) & Lm) << lgL) + x];
+        bad += (abs(c - r) > N) + (abs(c - d) > N);
+    }
+    for (int o = 16; o; o >>= 1) bad += __shfl_xor_sync(0xFFFFFFFFu, bad, o);
+    if ((threadIdx.x & 31) == 0 && bad) atomicAdd(d_bad, (unsigned long long)bad);
+}
+
+cudaError_t launch_violations(const int32_t *h, uint32_t L, uint32_t lgL, uint32_t nr, uint32_t N, unsigned long long *d_bad,
+                              cudaStream_t st)
+{
+    cudaError_t e = cudaMemsetAsync(d_bad, 0, sizeof(unsigned long long), st);
+    if (e != cudaSuccess) return e;
+    const uint64_t n = (uint64_t)L * L;
+    const uint32_t bx = (uint32_t)((n + RED_THREADS * 8 - 1) / (RED_THREADS * 8) < 2048 ? (n + RED_THREADS * 8 - 1) / (RED_THREADS * 8) : 2048);
+    for (uint32_t r0 = 0; r0 < nr; r0 += 65535) {
+        const uint32_t cnt = nr - r0 < 65535 ? nr - r0 : 65535;
+        violations_kernel<<<dim3(bx ? bx : 1, cnt), RED_THREADS, 0, st>>>(h + (size_t)r0 * n, L, lgL, (int32_t)N, d_bad);
+    }
+    return cudaGetLastError();
+}
+
 }  // namespace rsos

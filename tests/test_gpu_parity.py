@@ -434,3 +434,22 @@ def test_growth_exponent_sanity_c2(rsos):
     g.close()
     slope = np.polyfit(np.log(ts), np.log(w), 1)[0]
     assert 0.45 < slope < 0.50, slope
+
+
+def test_set_state_rejects_surfaces_that_violate_eq6(rsos):
+    """rsos_set_state checks Eq. (6) on the device (all engines rely on it): one bad bond -> RSOS_EINVAL."""
+    for engine in (rsos.ENGINE_THREAD, rsos.ENGINE_WARP):
+        g = rsos.Rsos(256, 2, 3, 1, engine=engine)
+        g.advance(2)
+        h = g.heights()
+        acc = g.sums()[2]
+        g.set_state(h, 2, acc)                              # its own state: fine
+        bad = h.copy()
+        bad[1, 17, 255] += 3                                # wraps to column 0: periodic bonds are checked too
+        with pytest.raises(rsos.RsosError) as e:
+            g.set_state(bad, 2, acc)
+        assert e.value.code == -1 and "Eq. (6)" in str(e.value)
+        g.set_state(h, 2, acc)                              # recover
+        g.advance(1)
+        assert (g.sums()[0] == g.sums()[2]).all()
+        g.close()
