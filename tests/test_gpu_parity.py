@@ -453,3 +453,50 @@ def test_set_state_rejects_surfaces_that_violate_eq6(rsos):
         g.advance(1)
         assert (g.sums()[0] == g.sums()[2]).all()
         g.close()
+
+
+def test_random_shapes_all_dt_engines(rsos, oracle_mod):
+    """Seeded random sweep over (L, N, R, S, K, engine, lanes): every DT engine against the oracle."""
+    rng = np.random.default_rng(20261104)
+    done = 0
+    while done < 24:
+        S = int(rng.choice([8, 16, 32, 64]))
+        L = int(S * rng.choice([2, 4, 8]))
+        if L > 512:
+            continue
+        K = int(rng.choice([k for k in (1, 2, 4, 8, 16) if S * S // k >= 32]))
+        N = int(rng.choice([1, 1, 2, 3, 5, 7]))
+        R = int(rng.integers(1, 6))
+        seed = int(rng.integers(1, 2 ** 40))
+        first = int(rng.integers(0, 1000))
+        lanes = int(rng.choice([l for l in (1, 2, 4, 8) if 8 * l <= S * S // K]))
+        engines = [(rsos.ENGINE_THREAD, lanes), (rsos.ENGINE_WARP, 0)]
+        o = oracle_mod.Oracle(L, N, R, seed, tile=S, subsweeps=K, first_real=first)
+        o.advance(3)
+        for eng, ln in engines:
+            g = rsos.Rsos(L, N, R, seed, tile=S, subsweeps=K, first_real=first, engine=eng, lanes=ln)
+            g.advance(1)
+            g.advance(2)
+            compare(g, o, "random L=%d N=%d R=%d S=%d K=%d engine=%d lanes=%d" % (L, N, R, S, K, eng, ln))
+            g.close()
+        o.close()
+        done += 1
+
+
+def test_largest_lattice_properties(rsos):
+    """L = 65536 (the largest the ABI accepts; 2^32 sites, 16 GiB of int32 heights, 1 GiB packed): what holds at any
+    size.  sum h = accepted; <h>(t=1) and W^2(t=1) are local quantities, so they must equal the DT(64,1) values of
+    the L = 128 ensemble of DESIGN.md section 12 (0.26587, 0.6516) -- here to 4e-4 relative (2^32 sites self-average)."""
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    if free < 24 * 2 ** 30:
+        pytest.skip("needs 24 GiB of device memory")
+    g = rsos.Rsos(65536, 1, 1, 7)
+    info = g.info()
+    assert info["engine"] == "thread" and info["blocks"] == 65536 * 4 * info["lanes"] // 32 * 1
+    g.advance(1)
+    s1, s2, acc = g.sums()
+    assert s1[0] == acc[0] and 0 < acc[0] <= 2 ** 32
+    w2, hm = g.width()
+    assert abs(w2[0] / 0.265867 - 1) < 4e-4 and abs(hm[0] / (0.65226 * (1 - 0.00101)) - 1) < 4e-4, (w2, hm)
+    g.close()
