@@ -4,18 +4,21 @@
 // Citations: P:n = PAPER.md line n; D:x = DESIGN.md section x.
 //
 // One colour pass of one sub-sweep (D:2 steps 4-6; RSOS rule P:61-63 Eq. 6; double tiling with a
-// moving origin P:77; independent realizations P:75).  Every THREAD owns one active tile and runs
-// its S*S/K attempts strictly in order, so the result is the sequential one by construction --
-// no speculation, no votes.  What makes that fast (D:4, D:5):
+// moving origin P:77; independent realizations P:75).  A tile is owned by KL = 1, 2, 4 or 8 lanes of
+// one warp (32 / KL tiles per warp) that run its S*S/K attempts in order, KL at a time; the result
+// is the sequential one (one lane: by construction; more lanes: a lane whose site clashes with a
+// lower rank's waits for it, see Attempt / group_finish).  What makes that fast (D:4, D:5):
 //   * a site is FB bits, its height mod 2^FB (FB = 2 for N = 1, FB = 4 for N <= 7): under Eq. (6)
 //     nearest-neighbour differences lie in [-N, N] and are recoverable mod 2^FB.  The working
 //     lattice in HBM is packed the same way (rsos_pack.cu), so a tile window is (S+2) rows of
 //     PW + 1 words instead of 4 bytes per site, and the int32 heights are rebuilt only on demand;
-//   * the window of a lane is stored word-interleaved, word w of lane l at smem[w * 32 + l]: a
-//     lane only ever touches bank l, so every shared-memory access of the attempt loop is
-//     conflict-free (one wavefront per warp instruction);
+//   * the windows of a warp are stored word-interleaved, word w of tile g at smem[w * NT + g]
+//     (NT = 32 / KL): lanes of different tiles never share a bank, and with one lane per tile every
+//     shared-memory access of the attempt loop is conflict-free;
 //   * window column 0 is the left halo (the packed row is funnel-shifted while staging), so the
-//     attempt loop has no per-tile alignment term.
+//     attempt loop has no per-tile alignment term;
+//   * fields are compared in the top bits of a register and moved there by multiplies, which run
+//     on the fma pipe; the integer alu pipe is what the loop saturates first (D:6).
 #include "rsos_device.cuh"
 #include "rsos_internal.h"
 

@@ -2,7 +2,7 @@
 //
 // Citations: P:n = PAPER.md line n; D:x = DESIGN.md section x.
 //
-// Three engines, all executing the seeded schedule of D:2 (RSOS rule P:61-63 Eq. 6, double tiling
+// Three of the four engines (the lane-per-tile THREAD engine lives in rsos_thread.cu), all executing the seeded schedule of D:2 (RSOS rule P:61-63 Eq. 6, double tiling
 // with a moving origin P:77, independent realizations P:75) and producing identical heights:
 //
 //   simple_*   one THREAD per active tile, heights in global memory, the literal loop nest.
