@@ -142,8 +142,10 @@ int rsos_get_heights(rsos_ctx *ctx, uint32_t r0, uint32_t nr, int32_t *host_out)
  * (host, nr int64).  For snapshot restarts: t enters the Philox counter, so (heights, t) is the
  * whole state.  Synchronises the stream.  Every engine relies on Eq. (6), so the written surfaces
  * are checked on the device: if some bond has |dh| > N the call returns RSOS_EINVAL -- the one
- * failure WITH an effect: the realizations hold host_in and t is set, and a valid state must be
- * set before the next rsos_advance.
+ * failure WITH an effect: the realizations hold host_in and t is set, and the context is marked
+ * invalid: rsos_advance, rsos_sums, rsos_width, rsos_moments and rsos_get_heights fail with
+ * RSOS_EINVAL until a later rsos_set_state leaves every surface of the context valid (while the
+ * mark is set, rsos_set_state checks the whole lattice, not only what it wrote).
  */
 int rsos_set_state(rsos_ctx *ctx, uint32_t r0, uint32_t nr, const int32_t *host_in,
                    uint64_t t, const int64_t *accepted);
@@ -172,14 +174,17 @@ int rsos_device_heights(rsos_ctx *ctx, int32_t **d);
 /*
  * rsos_kernel_time -- accumulated device time of the update kernels, measured with CUDA events on
  * the context's stream when timing was enabled with enable != 0 (it then records two events
- * around every rsos_advance).  Synchronises the stream.  *ms_total and *n_launches (host) receive
- * the totals since timing was enabled; enable = 0 switches it off.  Either pointer may be NULL.
+ * around the update launches of every rsos_advance; conversions between the packed and the int32
+ * lattice and the width kernels lie outside them).  Synchronises the stream.  *ms_total and
+ * *n_launches (host) receive the time and the number of update-kernel launches since timing was
+ * enabled; enable = 0 switches it off.  Either pointer may be NULL.
  */
 int rsos_kernel_time(rsos_ctx *ctx, int enable, double *ms_total, uint64_t *n_launches);
 
 /*
  * rsos_plan -- what rsos_init would choose for (L, N, R, opts) on a device with sm_count SMs
- * (<= 0: 148, a B200): pure host logic, needs no CUDA device.  out (host, 8 uint64): out[0] = mode
+ * (<= 0: the current CUDA device's count, or 148 -- a B200 -- when there is no device): pure host
+ * logic, needs no CUDA device.  out (host, 8 uint64): out[0] = mode
  * (0 RS, 1 DT), out[1] = engine, out[2] = S, out[3] = K, out[4] = active tiles per colour pass
  * (0 in RS mode), out[5] = THREAD engine lanes per tile (else 0), out[6] = bits per site of the
  * packed lattice (else 0), out[7] = kernel launches per MCS.  Same argument errors as rsos_init.

@@ -24,7 +24,8 @@
  * Pins (tests/test_oracle_*.py, all CPU): Eq. (6) invariant after every attempt, monotone
  * heights, sum h == accepted, random-deposition closed form, exact Markov-chain enumeration
  * on 2x2 / 4x4 (+3x3 through the general-L draw), Philox known answers + cuRAND header,
- * DT-vs-RS statistical agreement, tile-order independence, W2 recomputed with rationals.
+ * DT-vs-RS statistical agreement, tile-order independence, W2 recomputed with rationals;
+ * moments (Eq. 13-15): hand-worked 2x2 examples, scipy.stats, exact rationals.
  * "Parity unpinned": the schedule's free choices (S, colour order, slot layout, origin range)
  * cannot be pinned by the paper; they are pinned by oracle == GPU equality plus the
  * DT-vs-RS statistical test only.
@@ -371,3 +372,60 @@ int rsos_oracle_set_state(rsos_oracle *c, uint32_t r0, uint32_t nr, const int32_
 
 uint64_t rsos_oracle_time(const rsos_oracle *c) { return c->t; }
 int32_t *rsos_oracle_heights_ptr(rsos_oracle *c) { return c->h; }
+
+/* ------------------------------------------------------------------------------------------
+ * Moments of the height distribution of ONE surface.  Eq. (13) P:180-184 with the observable
+ * phi = h(x) and P_L the empirical distribution of the L*L heights of realization r:
+ *     hbar   = (1/L^2) sum_x h(x)
+ *     Phi^n  = (1/L^2) sum_x (h(x) - hbar)^n ,   n = 2, 3, 4
+ * written out as the definition: two passes in floating point (long double accumulators), no
+ * algebraic expansion into raw power sums.  out[0..2] = Phi^2, Phi^3, Phi^4; *hbar_out = hbar.
+ * The skewness Eq. (14) and kurtosis Eq. (15) of an ensemble are
+ *     S = <Phi^3> / <Phi^2>^(3/2),   Q = <Phi^4> / <Phi^2>^2 - 3
+ * with <.> the average over surfaces (and times) -- formed by the caller from these values.
+ * Pins (tests/test_oracle_moments.py): hand-worked 2x2 examples, scipy.stats moment/skew/kurtosis.
+ * ------------------------------------------------------------------------------------------ */
+int rsos_oracle_height_moments(const rsos_oracle *c, uint32_t r, double out[3], double *hbar_out)
+{
+    if (r >= c->R) return -1;
+    const size_t n = (size_t)c->L * c->L;
+    const int32_t *h = c->h + (size_t)r * n;
+    long double s = 0.0L;
+    for (size_t i = 0; i < n; ++i) s += (long double)h[i];
+    const long double hbar = s / (long double)n;
+    long double p2 = 0.0L, p3 = 0.0L, p4 = 0.0L;
+    for (size_t i = 0; i < n; ++i) {
+        const long double d = (long double)h[i] - hbar;
+        p2 += d * d;
+        p3 += d * d * d;
+        p4 += d * d * d * d;
+    }
+    out[0] = (double)(p2 / (long double)n);
+    out[1] = (double)(p3 / (long double)n);
+    out[2] = (double)(p4 / (long double)n);
+    if (hbar_out) *hbar_out = (double)hbar;
+    return 0;
+}
+
+/* Exact integer power sums about an integer base b:  M_k = sum_x (h(x) - b)^k, k = 1..4, as signed
+ * 128-bit integers, each written as two uint64 words (lo, hi).  This is the quantity the C ABI's
+ * rsos_moments returns (with b = floor(S1 / L^2)); the definition written out, one site at a time. */
+int rsos_oracle_power_sums(const rsos_oracle *c, uint32_t r, int64_t base, uint64_t out[8])
+{
+    if (r >= c->R) return -1;
+    const size_t n = (size_t)c->L * c->L;
+    const int32_t *h = c->h + (size_t)r * n;
+    __int128 m[4] = { 0, 0, 0, 0 };
+    for (size_t i = 0; i < n; ++i) {
+        const __int128 d = (__int128)h[i] - (__int128)base;
+        m[0] += d;
+        m[1] += d * d;
+        m[2] += d * d * d;
+        m[3] += d * d * d * d;
+    }
+    for (int k = 0; k < 4; ++k) {
+        out[2 * k] = (uint64_t)(unsigned __int128)m[k];
+        out[2 * k + 1] = (uint64_t)((unsigned __int128)m[k] >> 64);
+    }
+    return 0;
+}

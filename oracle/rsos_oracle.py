@@ -65,6 +65,10 @@ def lib():
         l.rsos_oracle_time.argtypes = [vp]
         l.rsos_oracle_time.restype = u64
         l.rsos_oracle_last_error.restype = C.c_char_p
+        l.rsos_oracle_height_moments.argtypes = [vp, u32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        l.rsos_oracle_height_moments.restype = C.c_int
+        l.rsos_oracle_power_sums.argtypes = [vp, u32, i64, C.POINTER(u64)]
+        l.rsos_oracle_power_sums.restype = C.c_int
         _lib = l
     return _lib
 
@@ -151,6 +155,25 @@ class Oracle:
         if self._l.rsos_oracle_set_state(self._c, r0, heights.shape[0], heights.ctypes.data, int(t),
                                          None if acc is None else acc.ctypes.data) != 0:
             raise ValueError("bad realization range")
+
+    def height_moments(self, r):
+        """(hbar, [Phi^2, Phi^3, Phi^4]) of the heights of realization r: Eq. (13) by definition."""
+        out = (C.c_double * 3)()
+        hb = C.c_double()
+        if self._l.rsos_oracle_height_moments(self._c, int(r), out, C.byref(hb)) != 0:
+            raise ValueError("bad realization")
+        return hb.value, [out[0], out[1], out[2]]
+
+    def power_sums(self, r, base):
+        """[M1..M4] with M_k = sum (h - base)^k as exact python ints."""
+        out = (C.c_uint64 * 8)()
+        if self._l.rsos_oracle_power_sums(self._c, int(r), int(base), out) != 0:
+            raise ValueError("bad realization")
+        res = []
+        for k in range(4):
+            v = int(out[2 * k]) | (int(out[2 * k + 1]) << 64)
+            res.append(v - (1 << 128) if v >> 127 else v)
+        return res
 
     def debug_violations(self):
         return self._l.rsos_oracle_debug_violations(self._c)

@@ -41,8 +41,11 @@ struct rsos_ctx {
     cudaEvent_t ev0, ev1;
     double ms_total;
     uint64_t timed_launches;
-    uint64_t launches_at_ev0;
+    uint64_t launches_at_ev0, launches_at_ev1;
     bool ev_pending;
+    // set by a rsos_set_state that wrote a surface violating Eq. (6); cleared by a set_state after which the
+    // whole lattice passes the check.  While set, every call that would run an engine or read sums fails.
+    bool state_invalid;
 };
 
 static thread_local char g_err[512] = "";
@@ -164,7 +167,17 @@ extern "C" int rsos_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts *o,
     memset(&opt, 0, sizeof opt);
     if (o) opt = *o;
     Plan pl;
-    const int rc = make_plan(L, N, R, opt, sm_count > 0 ? sm_count : 148, &pl);
+    if (sm_count <= 0) {                                   // the current device's SM count; 148 (a B200) without a device
+        int dev = 0, smc = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&smc, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && smc > 0)
+            sm_count = smc;
+        else {
+            cudaGetLastError();
+            sm_count = 148;
+        }
+    }
+    const int rc = make_plan(L, N, R, opt, sm_count, &pl);
     if (rc) return rc;
     out[0] = pl.mode_dt ? 1 : 0; out[1] = pl.engine; out[2] = pl.S; out[3] = pl.K;
     out[4] = pl.pass_tiles; out[5] = pl.lanes; out[6] = pl.field_bits;
@@ -181,8 +194,8 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
     if (o) opt = *o;
 
     Plan pl;
-    {   // argument errors are reported before any device is touched
-        const int rc0 = make_plan(L, N, R, opt, 148, &pl);
+    {   // argument errors are reported before any device is touched (the SM count only steers lanes per tile)
+        const int rc0 = make_plan(L, N, R, opt, 1, &pl);
         if (rc0) return rc0;
     }
     int dev = 0;
@@ -225,15 +238,17 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
     } while (0)
 
     const size_t bytes = (size_t)R * L * L * sizeof(int32_t);
+    const bool packed_state = engine == RSOS_ENGINE_THREAD;          // working state = packed lattice (D:5)
     if (opt.d_heights) { p.h = opt.d_heights; c->own_heights = false; }
-    else { INIT_TRY(cudaMalloc(&p.h, bytes), RSOS_ECUDA); c->own_heights = true; }
+    else if (!packed_state) { INIT_TRY(cudaMalloc(&p.h, bytes), RSOS_ECUDA); c->own_heights = true; }
+    // else: the int32 heights are allocated by the first call that needs them (alloc_heights)
     INIT_TRY(cudaMalloc(&p.accepted, (size_t)R * sizeof(unsigned long long)), RSOS_ECUDA);
     INIT_TRY(cudaMalloc(&p.err, sizeof(uint32_t)), RSOS_ECUDA);
     INIT_TRY(cudaMalloc(&c->d_red, (size_t)R * 8 * sizeof(unsigned long long)), RSOS_ECUDA);
     INIT_TRY(cudaMallocHost(&c->h_red, (size_t)R * 8 * sizeof(unsigned long long)), RSOS_ECUDA);
     INIT_TRY(cudaMalloc(&c->d_base, (size_t)R * sizeof(long long)), RSOS_ECUDA);
     c->h_valid = c->pk_valid = true;
-    if (engine == RSOS_ENGINE_THREAD) {
+    if (packed_state) {
         p.FB = pl.field_bits;
         p.KL = pl.lanes;
         const size_t pk_bytes = bytes / 32 * p.FB;                       // FB bits per site
@@ -246,7 +261,8 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
         INIT_TRY(cudaMemsetAsync(p.pk, 0, pk_bytes, c->stream), RSOS_ECUDA);                // flat start
         INIT_TRY(cudaMemsetAsync(c->d_s1off, 0, (size_t)R * sizeof(long long), c->stream), RSOS_ECUDA);
     }
-    INIT_TRY(cudaMemsetAsync(p.h, 0, bytes, c->stream), RSOS_ECUDA);                 // flat start
+    if (p.h) INIT_TRY(cudaMemsetAsync(p.h, 0, bytes, c->stream), RSOS_ECUDA);        // flat start
+    else c->h_valid = false;
     INIT_TRY(cudaMemsetAsync(p.accepted, 0, (size_t)R * sizeof(unsigned long long), c->stream), RSOS_ECUDA);
     INIT_TRY(cudaMemsetAsync(p.err, 0, sizeof(uint32_t), c->stream), RSOS_ECUDA);
     INIT_TRY(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev), RSOS_ECUDA);
@@ -276,9 +292,34 @@ static int flush_timing(rsos_ctx *c)
         float ms = 0.f;
         CUDA_TRY(cudaEventElapsedTime(&ms, c->ev0, c->ev1));
         c->ms_total += ms;
-        c->timed_launches += c->launches - c->launches_at_ev0;
+        c->timed_launches += c->launches_at_ev1 - c->launches_at_ev0;
         c->ev_pending = false;
     }
+    return RSOS_OK;
+}
+
+static int check_device_err(rsos_ctx *c)
+{
+    uint32_t e = 0;
+    CUDA_TRY(cudaMemcpyAsync(&e, c->p.err, sizeof e, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    if (e) return fail(RSOS_ECUDA, "device-side consistency check failed (flags 0x%x)", e);
+    return RSOS_OK;
+}
+
+// Packed working lattice (D:5): the int32 heights exist only once somebody asks for them.
+static int alloc_heights(rsos_ctx *c)
+{
+    if (c->p.h) return RSOS_OK;
+    const size_t bytes = (size_t)c->p.R * c->p.L * c->p.L * sizeof(int32_t);
+    const cudaError_t e = cudaMalloc(&c->p.h, bytes);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        c->p.h = nullptr;
+        return fail(e == cudaErrorMemoryAllocation ? RSOS_ENOMEM : RSOS_ECUDA, "int32 heights (%zu bytes): %s", bytes,
+                    cudaGetErrorString(e));
+    }
+    c->own_heights = true;
     return RSOS_OK;
 }
 
@@ -286,6 +327,10 @@ static int flush_timing(rsos_ctx *c)
 static int ensure_heights(rsos_ctx *c)
 {
     if (!c->p.pk || c->h_valid) return RSOS_OK;
+    {
+        const int rc = alloc_heights(c);
+        if (rc) return rc;
+    }
     uint32_t n = 0;
     CUDA_TRY(launch_unpack(c->p, c->d_s1off, c->d_V, c->d_srel, c->d_h00, c->stream, &n));
     c->launches += n;
@@ -298,7 +343,7 @@ static int ensure_packed(rsos_ctx *c)
 {
     if (!c->p.pk || c->pk_valid) return RSOS_OK;
     const Params &p = c->p;
-    CUDA_TRY(launch_sums(p.h, p.L, p.R, c->d_red, c->stream));
+    CUDA_TRY(launch_sums(p.h, p.L, p.R, c->d_red, c->sm_count, c->stream));
     CUDA_TRY(launch_s1off(p, c->d_red, c->d_s1off, c->stream));
     CUDA_TRY(launch_pack(p, c->stream));
     c->launches += (p.R + 65534) / 65535 + 2;
@@ -316,16 +361,17 @@ extern "C" int rsos_advance(rsos_ctx *c, uint64_t mcs)
                     (unsigned long long)mcs, p.K);
     DeviceGuard guard(c->device);
     if (!guard.ok) return fail(RSOS_ECUDA, "cannot select CUDA device %d", c->device);
-    if (c->timing) {
-        const int rc = flush_timing(c);
-        if (rc) return rc;
-        CUDA_TRY(cudaEventRecord(c->ev0, c->stream));
-        c->launches_at_ev0 = c->launches;
-    }
+    if (c->state_invalid) return fail(RSOS_EINVAL, "the state violates Eq. (6) (last rsos_set_state); set a valid state first");
     if (c->p.pk) {
         const int rc = ensure_packed(c);
         if (rc) return rc;
         c->h_valid = false;
+    }
+    if (c->timing) {                                       // the events bracket the update launches only
+        const int rc = flush_timing(c);
+        if (rc) return rc;
+        CUDA_TRY(cudaEventRecord(c->ev0, c->stream));
+        c->launches_at_ev0 = c->launches;
     }
     if (c->mode_dt) {
         for (uint64_t m = 0; m < mcs; ++m)
@@ -342,20 +388,13 @@ extern "C" int rsos_advance(rsos_ctx *c, uint64_t mcs)
     }
     if (c->timing) {
         CUDA_TRY(cudaEventRecord(c->ev1, c->stream));
+        c->launches_at_ev1 = c->launches;
         c->ev_pending = true;
     }
     c->t += mcs;
     return RSOS_OK;
 }
 
-static int check_device_err(rsos_ctx *c)
-{
-    uint32_t e = 0;
-    CUDA_TRY(cudaMemcpyAsync(&e, c->p.err, sizeof e, cudaMemcpyDeviceToHost, c->stream));
-    CUDA_TRY(cudaStreamSynchronize(c->stream));
-    if (e) return fail(RSOS_ECUDA, "device-side consistency check failed (flags 0x%x)", e);
-    return RSOS_OK;
-}
 
 // THREAD engine, packed lattice current: S1, S2 and max |h| straight from the packed lattice
 // (rsos_pack.cu): h = h00 + rel with h00 = (S1 - sum rel) / L^2 and S1 = s1off + accepted, so
@@ -396,11 +435,12 @@ static int reduce_sums_packed(rsos_ctx *c)
 static int reduce_sums(rsos_ctx *c)
 {
     const Params &p = c->p;
+    if (c->state_invalid) return fail(RSOS_EINVAL, "the state violates Eq. (6) (last rsos_set_state); set a valid state first");
     if (p.pk && !c->h_valid) {
         const int rc0 = reduce_sums_packed(c);
         if (rc0) return rc0;
     } else {
-        CUDA_TRY(launch_sums(p.h, p.L, p.R, c->d_red, c->stream));
+        CUDA_TRY(launch_sums(p.h, p.L, p.R, c->d_red, c->sm_count, c->stream));
         c->launches += (p.R + 65534) / 65535;
         CUDA_TRY(cudaMemcpyAsync(c->h_red, c->d_red, (size_t)p.R * 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost,
                                  c->stream));
@@ -462,6 +502,7 @@ extern "C" int rsos_moments(rsos_ctx *c, int64_t *base, uint64_t *out)
     if (!out) return fail(RSOS_EINVAL, "out is NULL");
     DeviceGuard guard(c->device);
     if (!guard.ok) return fail(RSOS_ECUDA, "cannot select CUDA device %d", c->device);
+    if (c->state_invalid) return fail(RSOS_EINVAL, "the state violates Eq. (6) (last rsos_set_state); set a valid state first");
     int rc = ensure_heights(c);                            // the moment kernel reads the int32 heights
     if (rc) return rc;
     rc = reduce_sums(c);
@@ -474,7 +515,7 @@ extern "C" int rsos_moments(rsos_ctx *c, int64_t *base, uint64_t *out)
         if (base) base[r] = hb[r];
     }
     CUDA_TRY(cudaMemcpyAsync(c->d_base, hb, (size_t)p.R * sizeof(long long), cudaMemcpyHostToDevice, c->stream));
-    CUDA_TRY(launch_moments(p.h, p.L, p.R, c->d_base, c->d_red, c->stream));
+    CUDA_TRY(launch_moments(p.h, p.L, p.R, c->d_base, c->d_red, c->sm_count, c->stream));
     c->launches += (p.R + 65534) / 65535;
     CUDA_TRY(cudaMemcpyAsync(out, c->d_red, (size_t)p.R * 8 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(cudaStreamSynchronize(c->stream));
@@ -488,6 +529,7 @@ extern "C" int rsos_get_heights(rsos_ctx *c, uint32_t r0, uint32_t nr, int32_t *
     if (nr && !host_out) return fail(RSOS_EINVAL, "host_out is NULL");
     DeviceGuard guard(c->device);
     if (!guard.ok) return fail(RSOS_ECUDA, "cannot select CUDA device %d", c->device);
+    if (c->state_invalid) return fail(RSOS_EINVAL, "the state violates Eq. (6) (last rsos_set_state); set a valid state first");
     {
         const int rc0 = ensure_heights(c);
         if (rc0) return rc0;
@@ -506,25 +548,41 @@ extern "C" int rsos_set_state(rsos_ctx *c, uint32_t r0, uint32_t nr, const int32
     if (t * c->p.K >= (1ull << 32)) return fail(RSOS_ERANGE, "t * K reaches 2^32");
     DeviceGuard guard(c->device);
     if (!guard.ok) return fail(RSOS_ECUDA, "cannot select CUDA device %d", c->device);
-    {
-        const int rc0 = ensure_heights(c);                 // realizations outside [r0, r0+nr) keep their state
-        if (rc0) return rc0;
+    if (c->p.pk) {
+        // realizations outside [r0, r0+nr) keep their state: bring the int32 copy up to date first.  When the whole
+        // lattice is overwritten (or already invalid) there is nothing to keep.
+        if (nr == c->p.R || c->state_invalid) {
+            const int rc0 = alloc_heights(c);
+            if (rc0) return rc0;
+        } else {
+            int rc0 = ensure_heights(c);
+            if (rc0) return rc0;
+            rc0 = check_device_err(c);                     // a failed reconstruction must not be handed on
+            if (rc0) return rc0;
+        }
+        c->h_valid = true;
         c->pk_valid = false;
     }
     const size_t per = (size_t)c->p.L * c->p.L;
     if (nr) CUDA_TRY(cudaMemcpyAsync(c->p.h + r0 * per, host_in, nr * per * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
     if (nr && accepted)
         CUDA_TRY(cudaMemcpyAsync(c->p.accepted + r0, accepted, nr * sizeof(int64_t), cudaMemcpyHostToDevice, c->stream));
-    if (nr) {                                              // every engine relies on Eq. (6): check what was written
-        CUDA_TRY(launch_violations(c->p.h + r0 * per, c->p.L, c->p.lgL, nr, c->p.N, c->d_red, c->stream));
+    c->t = t;
+    // Every engine relies on Eq. (6): check what was written -- and, while an earlier call left an invalid
+    // state behind, the whole lattice, so that the flag is only cleared when every surface is valid.
+    const uint32_t c0 = c->state_invalid ? 0u : r0, cn = c->state_invalid ? c->p.R : nr;
+    if (cn) {
+        CUDA_TRY(launch_violations(c->p.h + c0 * per, c->p.L, c->p.lgL, cn, c->p.N, c->d_red, c->stream));
         ++c->launches;
         CUDA_TRY(cudaMemcpyAsync(c->h_red, c->d_red, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
     }
     CUDA_TRY(cudaStreamSynchronize(c->stream));
-    c->t = t;
-    if (nr && c->h_red[0])
-        return fail(RSOS_EINVAL, "host_in violates Eq. (6) on %llu bonds (|dh| > N = %u); set a valid state before advancing",
+    if (cn && c->h_red[0]) {
+        c->state_invalid = true;
+        return fail(RSOS_EINVAL, "the written state violates Eq. (6) on %llu bonds (|dh| > N = %u); set a valid state before advancing",
                     c->h_red[0], c->p.N);
+    }
+    c->state_invalid = false;
     return RSOS_OK;
 }
 
@@ -557,7 +615,11 @@ extern "C" int rsos_device_heights(rsos_ctx *c, int32_t **d)
     {
         DeviceGuard guard(c->device);
         if (!guard.ok) return fail(RSOS_ECUDA, "cannot select CUDA device %d", c->device);
-        const int rc0 = ensure_heights(c);
+        int rc0 = alloc_heights(c);
+        if (rc0) return rc0;
+        rc0 = ensure_heights(c);
+        if (rc0) return rc0;
+        rc0 = check_device_err(c);                         // a failed reconstruction must not be handed out
         if (rc0) return rc0;
     }
     *d = c->p.h;

@@ -46,7 +46,7 @@ struct Params {
     uint32_t *err;                  // device error word (bit flags), see ERR_*
     uint32_t *pk;                   // THREAD engine: packed working lattice, FB bits per site (rsos_pack.cu)
     uint32_t FB;                    // field bits of pk (2 or 4); 0 when there is no packed lattice
-    uint32_t KL;                    // THREAD engine: lanes per tile (1, 2 or 4)
+    uint32_t KL;                    // THREAD engine: lanes per tile (1, 2, 4 or 8)
 };
 
 enum : uint32_t {

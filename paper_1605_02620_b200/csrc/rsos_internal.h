@@ -40,12 +40,12 @@ cudaError_t launch_unpack(const Params &p, const long long *d_s1off, int32_t *d_
 
 // rsos_reduce.cu
 // out: per realization 4 x uint64: S1 (as int64 bits), S2, max |h| (max over threads), unused
-cudaError_t launch_sums(const int32_t *h, uint32_t L, uint32_t R, unsigned long long *d_out, cudaStream_t st);
+cudaError_t launch_sums(const int32_t *h, uint32_t L, uint32_t R, unsigned long long *d_out, int sm_count, cudaStream_t st);
 // number of nearest-neighbour bonds with |dh| > N in nr surfaces (Eq. 6), added into *d_bad
 cudaError_t launch_violations(const int32_t *h, uint32_t L, uint32_t lgL, uint32_t nr, uint32_t N, unsigned long long *d_bad,
                               cudaStream_t st);
 // out: per realization 8 x uint64: M1..M4 as (lo, hi) two's-complement 128-bit
 cudaError_t launch_moments(const int32_t *h, uint32_t L, uint32_t R, const long long *d_base,
-                           unsigned long long *d_out, cudaStream_t st);
+                           unsigned long long *d_out, int sm_count, cudaStream_t st);
 
 }  // namespace rsos

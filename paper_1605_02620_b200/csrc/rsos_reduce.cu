@@ -53,14 +53,14 @@ __global__ void __launch_bounds__(RED_THREADS) sums_kernel(const int32_t *__rest
     }
 }
 
-cudaError_t launch_sums(const int32_t *h, uint32_t L, uint32_t R, unsigned long long *d_out, cudaStream_t st)
+cudaError_t launch_sums(const int32_t *h, uint32_t L, uint32_t R, unsigned long long *d_out, int sm_count, cudaStream_t st)
 {
     cudaError_t e = cudaMemsetAsync(d_out, 0, (size_t)R * 4 * sizeof(unsigned long long), st);
     if (e != cudaSuccess) return e;
     const uint64_t n4 = (uint64_t)L * L / 4;
-    // enough blocks per realization to cover 148 SMs x 8 blocks, at most one block per 256*4 int4
+    // enough blocks per realization to cover every SM with 8 blocks, at most one block per 256*4 int4
     uint64_t bx = (n4 + RED_THREADS * 4 - 1) / (RED_THREADS * 4);
-    const uint64_t want = (148 * 8 + R - 1) / R;
+    const uint64_t want = ((uint64_t)(sm_count > 0 ? sm_count : 1) * 8 + R - 1) / R;
     if (bx > want) bx = want;
     if (bx < 1) bx = 1;
     for (uint32_t r0 = 0; r0 < R; r0 += 65535) {
@@ -118,13 +118,13 @@ __global__ void __launch_bounds__(RED_THREADS) moments_kernel(const int32_t *__r
 }
 
 cudaError_t launch_moments(const int32_t *h, uint32_t L, uint32_t R, const long long *d_base,
-                           unsigned long long *d_out, cudaStream_t st)
+                           unsigned long long *d_out, int sm_count, cudaStream_t st)
 {
     cudaError_t e = cudaMemsetAsync(d_out, 0, (size_t)R * 8 * sizeof(unsigned long long), st);
     if (e != cudaSuccess) return e;
     const uint64_t n4 = (uint64_t)L * L / 4;
     uint64_t bx = (n4 + RED_THREADS * 4 - 1) / (RED_THREADS * 4);
-    const uint64_t want = (148 * 8 + R - 1) / R;
+    const uint64_t want = ((uint64_t)(sm_count > 0 ? sm_count : 1) * 8 + R - 1) / R;
     if (bx > want) bx = want;
     if (bx < 1) bx = 1;
     for (uint32_t r0 = 0; r0 < R; r0 += 65535) {

@@ -110,8 +110,9 @@ struct Geom {
 // ---------------------------------------------------------------------------------------------
 // All A attempts of one tile by one warp, exactly as if executed one after another (D:2 step 6).
 //
-// 32 consecutive attempts a0 .. a0+31 are in flight, attempt a on lane a & 31 (the slot layout of
-// D:2 makes each lane the owner of the Philox calls q = 32*c + lane, so it draws its own sites).
+// 32 consecutive attempts a0 .. a0+31 are in flight, attempt a on lane a & 31.  Attempt a takes the
+// 16-bit slot a & 7 of Philox call a >> 3 (D:2 step 6, reading Q16); lane l computes the calls
+// 32 g + l of every group g of 256 attempts and the slots reach their attempts through shuffles.
 // Window step (D:4):
 //   R  every lane reads the three words holding its 5-point stencil;
 //   D  decides on that snapshot: under Eq. (6) the deposit is rejected iff some neighbour

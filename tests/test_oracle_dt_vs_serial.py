@@ -35,7 +35,11 @@ def test_dt_matches_serial_rs(oracle_mod, S, K):
     standard errors at t = 10 and t = 100.  DT(64,1) (one origin per MCS, the paper's scheme verbatim,
     P:77) carries a known early-time bias of about -0.3 % in W2 that is unresolvable from t ~ 100 on
     (DESIGN.md "fidelity"): for it the 3-sigma test is applied at t = 100 and the t = 10
-    deviation is bounded by 0.6 % (far below the -3.5 % of 8x8 cells, checked by the next test)."""
+    deviation must lie in the band (-0.6 %, +0.1 %) around the measured bias of -0.24 % (DESIGN.md section 12;
+    combined SE here 0.09 %) -- far from the -3.5 % of 8x8 cells, which the next test checks is resolved.
+    This is a COARSE regression bound at fixed seeds (R = 1024 resolves 0.3 %, not 0.03 %): it ties the free
+    choices of the schedule to serial dynamics at that resolution and no finer; the high-precision bias
+    table (R = 4096 per schedule) is DESIGN.md section 12."""
     L, N, R, times = 128, 1, 1024, (10, 100)
     # serial dynamics at L = 128: a tile side > L/2 selects RS
     rs = run(oracle_mod, L, N, R, 128, 1, times, seed=101)
@@ -45,7 +49,8 @@ def test_dt_matches_serial_rs(oracle_mod, S, K):
         tol = 3.0 * np.sqrt(sem(a) ** 2 + sem(b) ** 2)
         assert tol < 0.02 * a.mean()                       # resolution: well below the 4 % bias of 8x8 cells
         if K == 1 and t < 100:
-            assert abs(a.mean() - b.mean()) <= 0.006 * a.mean(), (S, K, t, a.mean(), b.mean())
+            d = (b.mean() - a.mean()) / a.mean()
+            assert -0.006 < d < 0.001, (S, K, t, a.mean(), b.mean(), d)
         else:
             assert abs(a.mean() - b.mean()) <= tol, (S, K, t, a.mean(), b.mean(), tol)
         ha, hb = rs[t][1], dt[t][1]
