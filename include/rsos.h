@@ -50,8 +50,8 @@ enum {
 enum {
     RSOS_ENGINE_AUTO   = 0,  /* RS mode: ONCHIP when the lattice fits in shared memory, else      */
                              /* SIMPLE.  DT mode: THREAD when it applies and one colour pass has  */
-                             /* at least RSOS_THREAD_MIN_TILES active tiles, else WARP, else      */
-                             /* SIMPLE                                                            */
+                             /* at least RSOS_THREAD_MIN_TILES active tiles, else RESIDENT when   */
+                             /* it applies, else WARP, else SIMPLE                                */
     RSOS_ENGINE_SIMPLE = 1,  /* one thread per active tile, heights in global memory (slow;       */
                              /* the literal loop nest of D:2, kept as an on-device cross-check)   */
     RSOS_ENGINE_WARP   = 2,  /* DT mode: one warp per active tile, (S+2)^2 window staged in       */
@@ -59,9 +59,15 @@ enum {
                              /* needs tile <= 128 and N <= 31                                     */
     RSOS_ENGINE_ONCHIP = 3,  /* RS mode (2S > L): one warp per realization, the whole lattice     */
                              /* stays in shared memory for all MCS of one rsos_advance call       */
-    RSOS_ENGINE_THREAD = 4   /* DT mode: one thread per active tile, the tile window held in      */
+    RSOS_ENGINE_THREAD = 4,  /* DT mode: one thread per active tile, the tile window held in      */
                              /* bank-interleaved shared memory at 2 (N = 1) or 4 (N <= 7) bits    */
                              /* per site; needs tile <= 64 and N <= 7                             */
+    RSOS_ENGINE_RESIDENT = 5 /* DT mode, small lattices: one thread block per realization keeps   */
+                             /* the packed lattice in shared memory for every colour pass, sub-   */
+                             /* sweep and MCS of an rsos_advance call; 4..32 lanes per tile with  */
+                             /* exact hazard masks.  Needs 16 <= tile <= 64, N <= 7, at most 16   */
+                             /* tiles per colour pass of a realization (L <= 8 * tile) and        */
+                             /* tile^2 / subsweeps divisible by 8 * lanes                         */
 };
 #define RSOS_THREAD_MIN_TILES 4096u
 
@@ -80,9 +86,9 @@ typedef struct rsos_opts {
                           /* rsos_moments, rsos_set_state and rsos_device_heights.                */
     void    *stream;      /* cudaStream_t to enqueue on; NULL = the legacy default stream         */
     int32_t  device;      /* CUDA device ordinal + 1; 0 = the current device                      */
-    uint32_t lanes;       /* THREAD engine: lanes that share one tile, 1, 2, 4 or 8 (8 * lanes must not   */
-                          /* exceed tile^2 / subsweeps); 0 = chosen from the number of tiles per colour   */
-                          /* pass (D:4).  Does not change the result.                                     */
+    uint32_t lanes;       /* lanes that share one tile: THREAD engine 1, 2, 4 or 8, RESIDENT engine 4, 8, */
+                          /* 16 or 32 (8 * lanes must divide tile^2 / subsweeps); 0 = chosen by the       */
+                          /* library (D:4).  Does not change the result.                                  */
 } rsos_opts;
 
 /*
@@ -131,6 +137,18 @@ int rsos_width(rsos_ctx *ctx, double *W2, double *hmean);
 int rsos_moments(rsos_ctx *ctx, int64_t *base, uint64_t *out);
 
 /*
+ * rsos_height_moments -- central moments of the height distribution of each surface (Eq. 13, P:180-184,
+ * with the observable h(x) and the empirical distribution of the L*L sites of one realization):
+ *   hbar[r] = (1/L^2) sum_x h(x),   phi[r][n-2] = (1/L^2) sum_x (h(x) - hbar[r])^n  for n = 2, 3, 4.
+ * Formed on the host from the exact 128-bit power sums of rsos_moments (binomial expansion about the
+ * integer base, extended precision), so the only rounding is the final conversion to double.  The
+ * ensemble skewness / kurtosis of Eq. (14), (15) are <phi3> / <phi2>^(3/2) and <phi4> / <phi2>^2 - 3.
+ * Host buffers: hbar (R doubles, may be NULL), phi (R*3 doubles).  Synchronises the stream.
+ * Errors as rsos_moments.
+ */
+int rsos_height_moments(rsos_ctx *ctx, double *hbar, double *phi);
+
+/*
  * rsos_get_heights -- copy realizations r0 .. r0+nr-1 (nr*L*L int32, h[r][y][x]) to host_out.
  * Synchronises the stream.  Errors: RSOS_EINVAL if the range is outside [0, R), RSOS_ECUDA.
  */
@@ -157,8 +175,8 @@ int rsos_time(rsos_ctx *ctx, uint64_t *t);
  * rsos_info -- describe the context: out[0] = mode (0 RS, 1 DT), out[1] = engine in use,
  * out[2] = S (effective tile side), out[3] = K, out[4] = kernel launches enqueued so far,
  * out[5] = device SM count, out[6] = shared-memory bytes per block of the update kernel,
- * out[7] = update-kernel blocks per launch, out[8] = THREAD engine lanes per tile (else 0),
- * out[9] = bits per site of the packed working lattice (THREAD engine, else 0).
+ * out[7] = update-kernel blocks per launch, out[8] = lanes per tile (THREAD / RESIDENT, else 0),
+ * out[9] = bits per site of the packed working lattice (THREAD / RESIDENT engine, else 0).
  * Host buffer of 10 uint64.
  */
 int rsos_info(rsos_ctx *ctx, uint64_t *out);
@@ -186,8 +204,8 @@ int rsos_kernel_time(rsos_ctx *ctx, int enable, double *ms_total, uint64_t *n_la
  * (<= 0: the current CUDA device's count, or 148 -- a B200 -- when there is no device): pure host
  * logic, needs no CUDA device.  out (host, 8 uint64): out[0] = mode
  * (0 RS, 1 DT), out[1] = engine, out[2] = S, out[3] = K, out[4] = active tiles per colour pass
- * (0 in RS mode), out[5] = THREAD engine lanes per tile (else 0), out[6] = bits per site of the
- * packed lattice (else 0), out[7] = kernel launches per MCS.  Same argument errors as rsos_init.
+ * (0 in RS mode), out[5] = lanes per tile (THREAD / RESIDENT, else 0), out[6] = bits per site of the
+ * packed lattice (else 0), out[7] = kernel launches per MCS (RS mode and RESIDENT: per call).  Same argument errors as rsos_init.
  */
 int rsos_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts *opts, int sm_count, uint64_t *out);
 

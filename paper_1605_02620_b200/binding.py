@@ -12,12 +12,12 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "librsos.so")
 
-ENGINE_AUTO, ENGINE_SIMPLE, ENGINE_WARP, ENGINE_ONCHIP, ENGINE_THREAD = 0, 1, 2, 3, 4
-ENGINE_NAMES = {0: "auto", 1: "simple", 2: "warp", 3: "onchip", 4: "thread"}
+ENGINE_AUTO, ENGINE_SIMPLE, ENGINE_WARP, ENGINE_ONCHIP, ENGINE_THREAD, ENGINE_RESIDENT = 0, 1, 2, 3, 4, 5
+ENGINE_NAMES = {0: "auto", 1: "simple", 2: "warp", 3: "onchip", 4: "thread", 5: "resident"}
 RSOS_OK, RSOS_EINVAL, RSOS_ERANGE, RSOS_ENOMEM, RSOS_ECUDA, RSOS_EUNSUP = 0, -1, -2, -3, -4, -5
 
 # every symbol include/rsos.h declares (tests check the .so exports exactly these)
-SYMBOLS = ("rsos_init", "rsos_advance", "rsos_sums", "rsos_width", "rsos_moments", "rsos_get_heights",
+SYMBOLS = ("rsos_init", "rsos_advance", "rsos_sums", "rsos_width", "rsos_moments", "rsos_height_moments", "rsos_get_heights",
            "rsos_set_state", "rsos_time", "rsos_info", "rsos_device_heights", "rsos_kernel_time",
            "rsos_free", "rsos_last_error", "rsos_philox", "rsos_plan")
 
@@ -51,6 +51,7 @@ def load():
     l.rsos_sums.argtypes = [vp, vp, vp, vp]
     l.rsos_width.argtypes = [vp, vp, vp]
     l.rsos_moments.argtypes = [vp, vp, vp]
+    l.rsos_height_moments.argtypes = [vp, vp, vp]
     l.rsos_get_heights.argtypes = [vp, u32, u32, vp]
     l.rsos_set_state.argtypes = [vp, u32, u32, vp, u64, vp]
     l.rsos_time.argtypes = [vp, C.POINTER(u64)]
@@ -148,6 +149,13 @@ class Rsos:
                 row.append(v - (1 << 128) if v >> 127 else v)
             M.append(row)
         return base, M
+
+    def height_moments(self):
+        """(hbar[R], phi[R,3]): mean height and the central moments Phi^2, Phi^3, Phi^4 of every surface (Eq. 13)."""
+        hbar = np.empty(self.R, dtype=np.float64)
+        phi = np.empty((self.R, 3), dtype=np.float64)
+        _check(self._l.rsos_height_moments(self._c, hbar.ctypes.data, phi.ctypes.data))
+        return hbar, phi
 
     def heights(self, r0=0, nr=None, out=None):
         nr = self.R - r0 if nr is None else nr

@@ -109,14 +109,16 @@ struct Plan {
     uint64_t pass_tiles;
 };
 
-static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, int sm_count, Plan *pl)
+constexpr size_t SMEM_LIMIT_SM100 = 227u * 1024u;        // opt-in shared memory per block on sm_100a (rsos_plan without a device)
+
+static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, int sm_count, size_t smem_limit, Plan *pl)
 {
     if (!is_pow2(L) || L < 4 || L > 65536) return fail(RSOS_EINVAL, "L = %u must be a power of two in [4, 65536]", L);
     if (N < 1 || N > 127) return fail(RSOS_EINVAL, "N = %u must be in [1, 127]", N);
     if (R < 1) return fail(RSOS_EINVAL, "R must be >= 1");
-    if (opt.lanes != 0 && opt.lanes != 1 && opt.lanes != 2 && opt.lanes != 4 && opt.lanes != 8)
-        return fail(RSOS_EINVAL, "opts.lanes = %u must be 0, 1, 2, 4 or 8", opt.lanes);
-    if (opt.engine > RSOS_ENGINE_THREAD) return fail(RSOS_EINVAL, "unknown engine %u", opt.engine);
+    if (opt.lanes != 0 && opt.lanes != 1 && opt.lanes != 2 && opt.lanes != 4 && opt.lanes != 8 && opt.lanes != 16 && opt.lanes != 32)
+        return fail(RSOS_EINVAL, "opts.lanes = %u must be 0, 1, 2, 4, 8, 16 or 32", opt.lanes);
+    if (opt.engine > RSOS_ENGINE_RESIDENT) return fail(RSOS_EINVAL, "unknown engine %u", opt.engine);
     uint32_t S = opt.tile ? opt.tile : 64, K = opt.subsweeps ? opt.subsweeps : 1;
     if (!is_pow2(S) || S < 8) return fail(RSOS_EINVAL, "tile = %u must be a power of two >= 8", S);
     if (!is_pow2(K)) return fail(RSOS_EINVAL, "subsweeps = %u must be a power of two", K);
@@ -136,11 +138,21 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
     const bool thread_ok = mode_dt && S <= 64 && N <= 7;
     const bool onchip_ok = !mode_dt && L <= 128 && N <= 31;
     const uint64_t pass_tiles = mode_dt ? (uint64_t)R * (L / S / 2) * (L / S / 2) : 0;
+    // RESIDENT: lanes per tile = opts.lanes, else the widest group the tile's attempt count and shared memory allow
+    uint32_t res_lanes = 0;
+    if (mode_dt) {
+        if (opt.lanes) { if (resident_ok(L, N, S, K, opt.lanes, smem_limit)) res_lanes = opt.lanes; }
+        else for (uint32_t kl = 32; kl >= 4 && !res_lanes; kl /= 2) if (resident_ok(L, N, S, K, kl, smem_limit)) res_lanes = kl;
+    }
     if (engine == RSOS_ENGINE_AUTO) {
         if (!mode_dt) engine = onchip_ok ? RSOS_ENGINE_ONCHIP : RSOS_ENGINE_SIMPLE;
-        else if (thread_ok && pass_tiles >= RSOS_THREAD_MIN_TILES) engine = RSOS_ENGINE_THREAD;
+        else if (thread_ok && pass_tiles >= RSOS_THREAD_MIN_TILES && (!opt.lanes || opt.lanes <= 8)) engine = RSOS_ENGINE_THREAD;
+        else if (res_lanes) engine = RSOS_ENGINE_RESIDENT;
         else engine = warp_ok ? RSOS_ENGINE_WARP : thread_ok ? RSOS_ENGINE_THREAD : RSOS_ENGINE_SIMPLE;
     }
+    if (engine == RSOS_ENGINE_RESIDENT && !res_lanes)
+        return fail(RSOS_EUNSUP, "engine RESIDENT needs DT mode, 16 <= tile <= 64, N <= 7, at most 16 tiles per colour pass of a "
+                                 "realization, tile^2 / subsweeps divisible by 8 * lanes (lanes 4, 8, 16 or 32), and the packed lattice in shared memory");
     if (engine == RSOS_ENGINE_WARP && !warp_ok)
         return fail(RSOS_EUNSUP, "engine WARP needs DT mode (2*tile <= L), tile <= 128 and N <= 31");
     if (engine == RSOS_ENGINE_THREAD && !thread_ok)
@@ -149,7 +161,12 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
         return fail(RSOS_EUNSUP, "engine ONCHIP needs RS mode (2*tile > L), L <= 128 and N <= 31");
     pl->mode_dt = mode_dt; pl->engine = engine; pl->S = S; pl->K = K; pl->pass_tiles = pass_tiles;
     pl->lanes = 0; pl->field_bits = 0;
+    if (engine == RSOS_ENGINE_RESIDENT) {
+        pl->field_bits = thread_dt_field_bits(N, S);
+        pl->lanes = res_lanes;
+    }
     if (engine == RSOS_ENGINE_THREAD) {
+        if (opt.lanes > 8) return fail(RSOS_EINVAL, "opts.lanes = %u: the THREAD engine takes 1, 2, 4 or 8", opt.lanes);
         pl->field_bits = thread_dt_field_bits(N, S);
         uint32_t kl = opt.lanes ? opt.lanes : thread_dt_lanes_per_tile(pass_tiles, sm_count, pl->field_bits);
         while (!opt.lanes && 8ull * kl > (uint64_t)S * S / K) kl /= 2;                       // a batch is 8 * lanes attempts
@@ -177,11 +194,11 @@ extern "C" int rsos_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts *o,
             sm_count = 148;
         }
     }
-    const int rc = make_plan(L, N, R, opt, sm_count, &pl);
+    const int rc = make_plan(L, N, R, opt, sm_count, SMEM_LIMIT_SM100, &pl);
     if (rc) return rc;
     out[0] = pl.mode_dt ? 1 : 0; out[1] = pl.engine; out[2] = pl.S; out[3] = pl.K;
     out[4] = pl.pass_tiles; out[5] = pl.lanes; out[6] = pl.field_bits;
-    out[7] = pl.mode_dt ? (uint64_t)4 * pl.K : 1;                                             // launches per MCS
+    out[7] = pl.engine == RSOS_ENGINE_RESIDENT ? 1 : pl.mode_dt ? (uint64_t)4 * pl.K : 1;      // launches per MCS (RESIDENT, RS: per call)
     return RSOS_OK;
 }
 
@@ -195,7 +212,7 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
 
     Plan pl;
     {   // argument errors are reported before any device is touched (the SM count only steers lanes per tile)
-        const int rc0 = make_plan(L, N, R, opt, 1, &pl);
+        const int rc0 = make_plan(L, N, R, opt, 1, SMEM_LIMIT_SM100, &pl);
         if (rc0) return rc0;
     }
     int dev = 0;
@@ -204,9 +221,10 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
     DeviceGuard guard(dev);
     if (!guard.ok) return fail(RSOS_ECUDA, "cannot select CUDA device %d", dev);
     {
-        int smc = 0;
+        int smc = 0, smem_optin = 0;
         CUDA_TRY(cudaDeviceGetAttribute(&smc, cudaDevAttrMultiProcessorCount, dev));
-        const int rc0 = make_plan(L, N, R, opt, smc, &pl);
+        CUDA_TRY(cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+        const int rc0 = make_plan(L, N, R, opt, smc, (size_t)smem_optin, &pl);
         if (rc0) return rc0;
     }
     const bool mode_dt = pl.mode_dt;
@@ -238,7 +256,7 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
     } while (0)
 
     const size_t bytes = (size_t)R * L * L * sizeof(int32_t);
-    const bool packed_state = engine == RSOS_ENGINE_THREAD;          // working state = packed lattice (D:5)
+    const bool packed_state = engine == RSOS_ENGINE_THREAD || engine == RSOS_ENGINE_RESIDENT;   // working state = packed lattice (D:5)
     if (opt.d_heights) { p.h = opt.d_heights; c->own_heights = false; }
     else if (!packed_state) { INIT_TRY(cudaMalloc(&p.h, bytes), RSOS_ECUDA); c->own_heights = true; }
     // else: the int32 heights are allocated by the first call that needs them (alloc_heights)
@@ -271,7 +289,7 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
     INIT_TRY(cudaEventCreate(&c->ev0), RSOS_ECUDA);
     INIT_TRY(cudaEventCreate(&c->ev1), RSOS_ECUDA);
     c->smem_bytes = engine == RSOS_ENGINE_WARP ? warp_dt_smem(p.lgS) : engine == RSOS_ENGINE_ONCHIP ? warp_rs_smem(p.lgL)
-                    : engine == RSOS_ENGINE_THREAD ? thread_dt_smem(p) : 0;
+                    : engine == RSOS_ENGINE_THREAD ? thread_dt_smem(p) : engine == RSOS_ENGINE_RESIDENT ? resident_smem(p) : 0;
 #undef INIT_TRY
     *out = c;
     return RSOS_OK;
@@ -373,7 +391,17 @@ extern "C" int rsos_advance(rsos_ctx *c, uint64_t mcs)
         CUDA_TRY(cudaEventRecord(c->ev0, c->stream));
         c->launches_at_ev0 = c->launches;
     }
-    if (c->mode_dt) {
+    if (c->engine == RSOS_ENGINE_RESIDENT) {
+        // all colour passes and sub-sweeps of many MCS inside one launch; long calls are cut into launches of
+        // about 2^36 attempts (a fraction of a second) so that the stream stays responsive
+        const uint64_t per_mcs = (uint64_t)p.R * p.L * p.L;
+        const uint64_t chunk = per_mcs >= (1ull << 36) ? 1 : (1ull << 36) / per_mcs;
+        for (uint64_t m = 0; m < mcs; m += chunk) {
+            const uint64_t n = mcs - m < chunk ? mcs - m : chunk;
+            CUDA_TRY(resident_launch(p, (uint32_t)(c->t + m), (uint32_t)n, c->stream));
+            ++c->launches;
+        }
+    } else if (c->mode_dt) {
         for (uint64_t m = 0; m < mcs; ++m)
             for (uint32_t k = 0; k < p.K; ++k) {
                 const uint32_t u = (uint32_t)((c->t + m) * p.K + k);
@@ -520,6 +548,35 @@ extern "C" int rsos_moments(rsos_ctx *c, int64_t *base, uint64_t *out)
     CUDA_TRY(cudaMemcpyAsync(out, c->d_red, (size_t)p.R * 8 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(cudaStreamSynchronize(c->stream));
     return RSOS_OK;
+}
+
+extern "C" int rsos_height_moments(rsos_ctx *c, double *hbar, double *phi)
+{
+    if (!c) return fail(RSOS_EINVAL, "ctx is NULL");
+    if (!phi) return fail(RSOS_EINVAL, "phi is NULL");
+    const uint32_t R = c->p.R;
+    uint64_t *raw = static_cast<uint64_t *>(malloc((size_t)R * 8 * sizeof(uint64_t)));
+    int64_t *base = static_cast<int64_t *>(malloc((size_t)R * sizeof(int64_t)));
+    if (!raw || !base) { free(raw); free(base); return fail(RSOS_ENOMEM, "out of host memory"); }
+    const int rc = rsos_moments(c, base, raw);
+    if (rc == RSOS_OK) {
+        const long double n = (long double)c->p.L * (long double)c->p.L;
+        for (uint32_t r = 0; r < R; ++r) {
+            long double a[4];
+            for (int k = 0; k < 4; ++k) {
+                const unsigned __int128 u = ((unsigned __int128)raw[8 * (size_t)r + 2 * k + 1] << 64) | raw[8 * (size_t)r + 2 * k];
+                a[k] = (long double)(__int128)u / n;       // raw moment about the integer base, per site
+            }
+            const long double m1 = a[0];                   // 0 <= m1 < 1: the base is floor(mean)
+            phi[3 * (size_t)r + 0] = (double)(a[1] - m1 * m1);
+            phi[3 * (size_t)r + 1] = (double)(a[2] - 3 * m1 * a[1] + 2 * m1 * m1 * m1);
+            phi[3 * (size_t)r + 2] = (double)(a[3] - 4 * m1 * a[2] + 6 * m1 * m1 * a[1] - 3 * m1 * m1 * m1 * m1);
+            if (hbar) hbar[r] = (double)((long double)base[r] + m1);
+        }
+    }
+    free(raw);
+    free(base);
+    return rc;
 }
 
 extern "C" int rsos_get_heights(rsos_ctx *c, uint32_t r0, uint32_t nr, int32_t *host_out)

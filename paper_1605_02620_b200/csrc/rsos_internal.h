@@ -12,7 +12,7 @@ struct Params;
 constexpr int WARP_DT_WARPS = 1;     // warps (= tiles) per block of the DT warp engine (1: even spread over SMs)
 constexpr int WARP_RS_WARPS = 4;     // warps (= realizations) per block of the on-chip RS engine
 
-enum : uint32_t { ENGINE_AUTO = 0, ENGINE_SIMPLE = 1, ENGINE_WARP = 2, ENGINE_ONCHIP = 3, ENGINE_THREAD = 4 };
+enum : uint32_t { ENGINE_AUTO = 0, ENGINE_SIMPLE = 1, ENGINE_WARP = 2, ENGINE_ONCHIP = 3, ENGINE_THREAD = 4, ENGINE_RESIDENT = 5 };
 
 // rsos_update.cu
 size_t warp_dt_smem(uint32_t lgS);
@@ -30,6 +30,13 @@ size_t thread_dt_smem(const Params &p);
 cudaError_t thread_dt_configure(const Params &p);
 uint32_t thread_dt_blocks(const Params &p);
 cudaError_t thread_dt_launch(const Params &p, uint32_t u, uint32_t colour, uint32_t blocks, cudaStream_t st);
+
+// rsos_resident.cu (DT schedule with the packed lattice resident in shared memory for a whole rsos_advance)
+bool resident_ok(uint32_t L, uint32_t N, uint32_t S, uint32_t K, uint32_t KL, size_t smem_limit);
+size_t resident_smem(const Params &p);
+cudaError_t resident_configure(const Params &p);
+uint32_t resident_blocks(const Params &p);
+cudaError_t resident_launch(const Params &p, uint32_t t0, uint32_t mcs, cudaStream_t st);
 
 // rsos_pack.cu (packed working lattice <-> int32 heights)
 cudaError_t launch_pack(const Params &p, cudaStream_t st);

@@ -116,6 +116,53 @@ def test_dt_thread_engine_equals_oracle(rsos, oracle_mod, L, N, R, S, K, mcs, se
     g.close()
 
 
+@pytest.mark.parametrize("L,N,R,S,K,mcs,seed", [
+    (128, 1, 3, 64, 1, 6, 1),        # one tile per colour pass and realization
+    (128, 1, 9, 64, 4, 5, 21),       # C5's shape at L = 128 (K = 4); with < 32 lanes several realizations share a block
+    (256, 1, 5, 64, 4, 4, 2),        # 4 tiles per pass: 4 warps (32 lanes) .. 1 warp (8 lanes) per block
+    (512, 1, 2, 64, 4, 3, 12),       # 16 tiles per pass, 64 KiB lattice
+    (256, 2, 2, 64, 4, 4, 3),        # 4-bit sites (N = 2)
+    (512, 2, 1, 64, 4, 2, 14),       # 128 KiB lattice
+    (256, 4, 1, 64, 1, 4, 4),
+    (256, 7, 1, 64, 2, 3, 5),        # largest N of the 4-bit format
+    (128, 1, 2, 32, 4, 5, 6),        # S = 32, A = 256: one batch at 32 lanes
+    (256, 3, 2, 32, 1, 3, 16),       # S = 32, 16 tiles per pass
+    (64, 2, 3, 16, 1, 5, 7),         # S = 16
+    (64, 1, 5, 16, 2, 5, 8),         # S = 16, 2-bit sites (a tile row is exactly one packed word)
+])
+@pytest.mark.parametrize("lanes", [4, 8, 16, 32])
+def test_dt_resident_engine_equals_oracle(rsos, oracle_mod, L, N, R, S, K, mcs, seed, lanes):
+    """The RESIDENT engine (packed lattice in shared memory across passes; MATCH-based hazard masks), 4 .. 32 lanes per tile."""
+    if (S * S // K) % (8 * lanes):
+        pytest.skip("a batch of 8 * lanes attempts does not divide the tile's attempts")
+    g = rsos.Rsos(L, N, R, seed, tile=S, subsweeps=K, engine=rsos.ENGINE_RESIDENT, lanes=lanes)
+    o = oracle_mod.Oracle(L, N, R, seed, tile=S, subsweeps=K)
+    info = g.info()
+    assert info["mode"] == "DT" and info["engine"] == "resident" and info["lanes"] == lanes, info
+    for step in (1, 1, mcs - 2):                            # single MCS and several MCS inside one launch
+        g.advance(step)
+        o.advance(step)
+        compare(g, o, "DT resident L=%d N=%d S=%d K=%d lanes=%d t=%d" % (L, N, S, K, lanes, g.t))
+    g.close()
+
+
+def test_dt_resident_engine_snapshot_restart(rsos, oracle_mod):
+    """RESIDENT engine: packed working state, heights read back mid-run, a partial rsos_set_state, many MCS per launch."""
+    L, N, R, seed = 128, 1, 6, 41
+    g = rsos.Rsos(L, N, R, seed, subsweeps=4)
+    assert g.info()["engine"] == "resident"
+    o = oracle_mod.Oracle(L, N, R, seed, subsweeps=4)
+    g.advance(40)
+    o.advance(40)
+    compare(g, o, "before snapshot")
+    h, acc = o.heights(), o.sums()[2]
+    g.set_state(h[2:4], 40, acc[2:4], r0=2)
+    g.advance(25)
+    o.advance(25)
+    compare(g, o, "after partial set_state")
+    g.close()
+
+
 @pytest.mark.parametrize("L,N,R,mcs", [(2048, 1, 2, 2),     # 512 tiles per pass; rows rebuilt by one warp each
                                        (4096, 1, 1, 1),     # 256 packed words per row: rows rebuilt by a whole block
                                        (2048, 3, 1, 1)])    # 4-bit sites, 256 words per row
@@ -471,6 +518,9 @@ def test_random_shapes_all_dt_engines(rsos, oracle_mod):
         first = int(rng.integers(0, 1000))
         lanes = int(rng.choice([l for l in (1, 2, 4, 8) if 8 * l <= S * S // K]))
         engines = [(rsos.ENGINE_THREAD, lanes), (rsos.ENGINE_WARP, 0)]
+        res_lanes = [l for l in (4, 8, 16, 32) if S >= 16 and L <= 8 * S and (S * S // K) % (8 * l) == 0]
+        if res_lanes:
+            engines.append((rsos.ENGINE_RESIDENT, int(rng.choice(res_lanes))))
         o = oracle_mod.Oracle(L, N, R, seed, tile=S, subsweeps=K, first_real=first)
         o.advance(3)
         for eng, ln in engines:
