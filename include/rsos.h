@@ -62,12 +62,12 @@ enum {
     RSOS_ENGINE_THREAD = 4,  /* DT mode: one thread per active tile, the tile window held in      */
                              /* bank-interleaved shared memory at 2 (N = 1) or 4 (N <= 7) bits    */
                              /* per site; needs tile <= 64 and N <= 7                             */
-    RSOS_ENGINE_RESIDENT = 5 /* DT mode, small lattices: one thread block per realization keeps   */
-                             /* the packed lattice in shared memory for every colour pass, sub-   */
-                             /* sweep and MCS of an rsos_advance call; 4..32 lanes per tile with  */
-                             /* exact hazard masks.  Needs 16 <= tile <= 64, N <= 7, at most 16   */
-                             /* tiles per colour pass of a realization (L <= 8 * tile) and        */
-                             /* tile^2 / subsweeps divisible by 8 * lanes                         */
+    RSOS_ENGINE_RESIDENT = 5 /* DT mode, small lattices: a cluster of thread blocks keeps the     */
+                             /* lattice of one realization in (distributed) shared memory for     */
+                             /* every colour pass, sub-sweep and MCS of an rsos_advance call; one */
+                             /* warp per tile, 32 attempts in flight with exact conflict votes.   */
+                             /* Needs 16 <= tile <= 64, N <= 7 and the lattice in the shared      */
+                             /* memory of at most 16 blocks (L <= 512 at N = 1)                   */
 };
 #define RSOS_THREAD_MIN_TILES 4096u
 
@@ -86,9 +86,13 @@ typedef struct rsos_opts {
                           /* rsos_moments, rsos_set_state and rsos_device_heights.                */
     void    *stream;      /* cudaStream_t to enqueue on; NULL = the legacy default stream         */
     int32_t  device;      /* CUDA device ordinal + 1; 0 = the current device                      */
-    uint32_t lanes;       /* lanes that share one tile: THREAD engine 1, 2, 4 or 8, RESIDENT engine 4, 8, */
-                          /* 16 or 32 (8 * lanes must divide tile^2 / subsweeps); 0 = chosen by the       */
-                          /* library (D:4).  Does not change the result.                                  */
+    uint32_t lanes;       /* THREAD engine: lanes that share one tile, 1, 2, 4 or 8 (8 * lanes must not   */
+                          /* exceed tile^2 / subsweeps); 0 = chosen from the number of tiles per colour   */
+                          /* pass (D:4).  Does not change the result.                                     */
+    uint32_t cluster;     /* RESIDENT engine: thread blocks per realization (a thread-block cluster that  */
+                          /* shares its shared memory), 1, 2, 4, 8 or 16; must divide the (L / 2 tile)^2  */
+                          /* tiles of a colour pass; 0 = chosen by the library.  Does not change the      */
+                          /* result.                                                                      */
 } rsos_opts;
 
 /*
@@ -176,8 +180,10 @@ int rsos_time(rsos_ctx *ctx, uint64_t *t);
  * out[2] = S (effective tile side), out[3] = K, out[4] = kernel launches enqueued so far,
  * out[5] = device SM count, out[6] = shared-memory bytes per block of the update kernel,
  * out[7] = update-kernel blocks per launch, out[8] = lanes per tile (THREAD / RESIDENT, else 0),
- * out[9] = bits per site of the packed working lattice (THREAD / RESIDENT engine, else 0).
- * Host buffer of 10 uint64.
+ * out[9] = bits per site of the packed working lattice (THREAD / RESIDENT engine, else 0),
+ * out[10] = RESIDENT engine blocks per cluster (else 0), out[11] = 1 if the int32 height buffer
+ * exists (it is allocated on first use when the working state is the packed lattice).
+ * Host buffer of 12 uint64.
  */
 int rsos_info(rsos_ctx *ctx, uint64_t *out);
 
@@ -202,10 +208,11 @@ int rsos_kernel_time(rsos_ctx *ctx, int enable, double *ms_total, uint64_t *n_la
 /*
  * rsos_plan -- what rsos_init would choose for (L, N, R, opts) on a device with sm_count SMs
  * (<= 0: the current CUDA device's count, or 148 -- a B200 -- when there is no device): pure host
- * logic, needs no CUDA device.  out (host, 8 uint64): out[0] = mode
+ * logic, needs no CUDA device.  out (host, 9 uint64): out[0] = mode
  * (0 RS, 1 DT), out[1] = engine, out[2] = S, out[3] = K, out[4] = active tiles per colour pass
  * (0 in RS mode), out[5] = lanes per tile (THREAD / RESIDENT, else 0), out[6] = bits per site of the
- * packed lattice (else 0), out[7] = kernel launches per MCS (RS mode and RESIDENT: per call).  Same argument errors as rsos_init.
+ * packed lattice (else 0), out[7] = kernel launches per MCS (RS mode and RESIDENT: per call),
+ * out[8] = RESIDENT engine blocks per cluster (else 0); out is 9 uint64.  Same argument errors as rsos_init.
  */
 int rsos_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts *opts, int sm_count, uint64_t *out);
 

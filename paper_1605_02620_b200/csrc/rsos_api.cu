@@ -105,7 +105,7 @@ static void destroy(rsos_ctx *c)
 // Shared by rsos_init and rsos_plan; needs no device.
 struct Plan {
     bool mode_dt;
-    uint32_t engine, S, K, lanes, field_bits;
+    uint32_t engine, S, K, lanes, field_bits, cluster;
     uint64_t pass_tiles;
 };
 
@@ -116,8 +116,10 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
     if (!is_pow2(L) || L < 4 || L > 65536) return fail(RSOS_EINVAL, "L = %u must be a power of two in [4, 65536]", L);
     if (N < 1 || N > 127) return fail(RSOS_EINVAL, "N = %u must be in [1, 127]", N);
     if (R < 1) return fail(RSOS_EINVAL, "R must be >= 1");
-    if (opt.lanes != 0 && opt.lanes != 1 && opt.lanes != 2 && opt.lanes != 4 && opt.lanes != 8 && opt.lanes != 16 && opt.lanes != 32)
-        return fail(RSOS_EINVAL, "opts.lanes = %u must be 0, 1, 2, 4, 8, 16 or 32", opt.lanes);
+    if (opt.lanes != 0 && opt.lanes != 1 && opt.lanes != 2 && opt.lanes != 4 && opt.lanes != 8)
+        return fail(RSOS_EINVAL, "opts.lanes = %u must be 0, 1, 2, 4 or 8", opt.lanes);
+    if (opt.cluster != 0 && opt.cluster != 1 && opt.cluster != 2 && opt.cluster != 4 && opt.cluster != 8 && opt.cluster != 16)
+        return fail(RSOS_EINVAL, "opts.cluster = %u must be 0, 1, 2, 4, 8 or 16", opt.cluster);
     if (opt.engine > RSOS_ENGINE_RESIDENT) return fail(RSOS_EINVAL, "unknown engine %u", opt.engine);
     uint32_t S = opt.tile ? opt.tile : 64, K = opt.subsweeps ? opt.subsweeps : 1;
     if (!is_pow2(S) || S < 8) return fail(RSOS_EINVAL, "tile = %u must be a power of two >= 8", S);
@@ -138,21 +140,22 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
     const bool thread_ok = mode_dt && S <= 64 && N <= 7;
     const bool onchip_ok = !mode_dt && L <= 128 && N <= 31;
     const uint64_t pass_tiles = mode_dt ? (uint64_t)R * (L / S / 2) * (L / S / 2) : 0;
-    // RESIDENT: lanes per tile = opts.lanes, else the widest group the tile's attempt count and shared memory allow
-    uint32_t res_lanes = 0;
+    // RESIDENT: blocks per cluster (= per realization) = opts.cluster, else chosen from the shared memory a block
+    // may use and the number of blocks the machine needs (rsos_resident.cu)
+    uint32_t res_cluster = 0;
     if (mode_dt) {
-        if (opt.lanes) { if (resident_ok(L, N, S, K, opt.lanes, smem_limit)) res_lanes = opt.lanes; }
-        else for (uint32_t kl = 32; kl >= 4 && !res_lanes; kl /= 2) if (resident_ok(L, N, S, K, kl, smem_limit)) res_lanes = kl;
+        if (opt.cluster) { if (resident_ok(L, N, S, K, opt.cluster, smem_limit)) res_cluster = opt.cluster; }
+        else res_cluster = resident_cluster_size(L, N, S, K, R, sm_count, smem_limit);
     }
     if (engine == RSOS_ENGINE_AUTO) {
         if (!mode_dt) engine = onchip_ok ? RSOS_ENGINE_ONCHIP : RSOS_ENGINE_SIMPLE;
-        else if (thread_ok && pass_tiles >= RSOS_THREAD_MIN_TILES && (!opt.lanes || opt.lanes <= 8)) engine = RSOS_ENGINE_THREAD;
-        else if (res_lanes) engine = RSOS_ENGINE_RESIDENT;
+        else if (thread_ok && pass_tiles >= RSOS_THREAD_MIN_TILES) engine = RSOS_ENGINE_THREAD;
+        else if (res_cluster && pass_tiles / R <= 16) engine = RSOS_ENGINE_RESIDENT;   // few tiles per pass and realization
         else engine = warp_ok ? RSOS_ENGINE_WARP : thread_ok ? RSOS_ENGINE_THREAD : RSOS_ENGINE_SIMPLE;
     }
-    if (engine == RSOS_ENGINE_RESIDENT && !res_lanes)
-        return fail(RSOS_EUNSUP, "engine RESIDENT needs DT mode, 16 <= tile <= 64, N <= 7, at most 16 tiles per colour pass of a "
-                                 "realization, tile^2 / subsweeps divisible by 8 * lanes (lanes 4, 8, 16 or 32), and the packed lattice in shared memory");
+    if (engine == RSOS_ENGINE_RESIDENT && !res_cluster)
+        return fail(RSOS_EUNSUP, "engine RESIDENT needs DT mode, 16 <= tile <= 64, N <= 7, a cluster size of 1, 2, 4, 8 or 16 that divides "
+                                 "the (L / 2 tile)^2 tiles of a colour pass with at most 16 tiles per block, and the lattice slab in shared memory");
     if (engine == RSOS_ENGINE_WARP && !warp_ok)
         return fail(RSOS_EUNSUP, "engine WARP needs DT mode (2*tile <= L), tile <= 128 and N <= 31");
     if (engine == RSOS_ENGINE_THREAD && !thread_ok)
@@ -161,12 +164,13 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
         return fail(RSOS_EUNSUP, "engine ONCHIP needs RS mode (2*tile > L), L <= 128 and N <= 31");
     pl->mode_dt = mode_dt; pl->engine = engine; pl->S = S; pl->K = K; pl->pass_tiles = pass_tiles;
     pl->lanes = 0; pl->field_bits = 0;
+    pl->cluster = 0;
     if (engine == RSOS_ENGINE_RESIDENT) {
         pl->field_bits = thread_dt_field_bits(N, S);
-        pl->lanes = res_lanes;
+        pl->lanes = 32;                                    // one warp per tile
+        pl->cluster = res_cluster;
     }
     if (engine == RSOS_ENGINE_THREAD) {
-        if (opt.lanes > 8) return fail(RSOS_EINVAL, "opts.lanes = %u: the THREAD engine takes 1, 2, 4 or 8", opt.lanes);
         pl->field_bits = thread_dt_field_bits(N, S);
         uint32_t kl = opt.lanes ? opt.lanes : thread_dt_lanes_per_tile(pass_tiles, sm_count, pl->field_bits);
         while (!opt.lanes && 8ull * kl > (uint64_t)S * S / K) kl /= 2;                       // a batch is 8 * lanes attempts
@@ -199,6 +203,7 @@ extern "C" int rsos_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts *o,
     out[0] = pl.mode_dt ? 1 : 0; out[1] = pl.engine; out[2] = pl.S; out[3] = pl.K;
     out[4] = pl.pass_tiles; out[5] = pl.lanes; out[6] = pl.field_bits;
     out[7] = pl.engine == RSOS_ENGINE_RESIDENT ? 1 : pl.mode_dt ? (uint64_t)4 * pl.K : 1;      // launches per MCS (RESIDENT, RS: per call)
+    out[8] = pl.cluster;
     return RSOS_OK;
 }
 
@@ -269,6 +274,7 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
     if (packed_state) {
         p.FB = pl.field_bits;
         p.KL = pl.lanes;
+        p.CS = pl.cluster;
         const size_t pk_bytes = bytes / 32 * p.FB;                       // FB bits per site
         INIT_TRY(cudaMalloc(&p.pk, pk_bytes), RSOS_ECUDA);
         INIT_TRY(cudaMalloc(&c->d_s1off, (size_t)R * sizeof(long long)), RSOS_ECUDA);
@@ -663,6 +669,8 @@ extern "C" int rsos_info(rsos_ctx *c, uint64_t *out)
     out[7] = c->blocks;
     out[8] = c->p.pk ? c->p.KL : 0;
     out[9] = c->p.pk ? c->p.FB : 0;
+    out[10] = c->engine == RSOS_ENGINE_RESIDENT ? c->p.CS : 0;
+    out[11] = c->p.h ? 1 : 0;
     return RSOS_OK;
 }
 

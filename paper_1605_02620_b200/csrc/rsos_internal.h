@@ -32,7 +32,8 @@ uint32_t thread_dt_blocks(const Params &p);
 cudaError_t thread_dt_launch(const Params &p, uint32_t u, uint32_t colour, uint32_t blocks, cudaStream_t st);
 
 // rsos_resident.cu (DT schedule with the packed lattice resident in shared memory for a whole rsos_advance)
-bool resident_ok(uint32_t L, uint32_t N, uint32_t S, uint32_t K, uint32_t KL, size_t smem_limit);
+bool resident_ok(uint32_t L, uint32_t N, uint32_t S, uint32_t K, uint32_t csize, size_t smem_limit);
+uint32_t resident_cluster_size(uint32_t L, uint32_t N, uint32_t S, uint32_t K, uint32_t R, int sm_count, size_t smem_limit);
 size_t resident_smem(const Params &p);
 cudaError_t resident_configure(const Params &p);
 uint32_t resident_blocks(const Params &p);

@@ -99,8 +99,18 @@ def test_plan_picks_engines_lanes_and_site_width(lib_path):
     assert (p["engine"], p["lanes"], p["packed_bits"]) == ("thread", 4, 4)         # 4-bit sites for N = 2..7
     p = m.plan(c["C4"]["L"], 1, 1)
     assert (p["engine"], p["pass_tiles"], p["lanes"], p["launches_per_mcs"]) == ("thread", 65536, 2, 4)
-    p = m.plan(128, 1, w.c5_realizations(128), tile=64, subsweeps=4)                  # C5 at L = 128: few tiles per pass
-    assert (p["engine"], p["pass_tiles"], p["launches_per_mcs"]) == ("warp", 1024, 16)
+    for L, cl in ((128, 1), (256, 1), (512, 2)):                                      # C5: few tiles per pass -> lattice on chip
+        for N in (1, 2):
+            p = m.plan(L, N, w.c5_realizations(L), tile=64, subsweeps=4)
+            assert (p["engine"], p["pass_tiles"], p["launches_per_mcs"], p["cluster"], p["lanes"], p["packed_bits"]) == \
+                ("resident", 1024, 1, cl, 32, 2 * N), (L, N, p)
+    assert m.plan(512, 1, 64, tile=64, subsweeps=4, cluster=8)["cluster"] == 8        # any cluster size that divides the 16 tiles
+    with pytest.raises(m.RsosError) as e:
+        m.plan(512, 1, 64, tile=64, subsweeps=4, engine=m.ENGINE_RESIDENT, cluster=1) # 256 KiB of uint8 sites do not
+    assert e.value.code == -5
+    p = m.plan(128, 1, 1024, tile=64, subsweeps=4, engine=m.ENGINE_WARP)
+    assert (p["engine"], p["launches_per_mcs"]) == ("warp", 16)
+    assert m.plan(2048, 1, 1)["engine"] == "warp"                                    # 256 tiles per pass: not resident, too few for THREAD
     assert m.plan(64, 1, 4096)["engine"] == "onchip" and m.plan(512, 1, 2, tile=512)["engine"] == "simple"
     assert m.plan(256, 8, 4096)["engine"] == "warp" and m.plan(256, 40, 4096)["engine"] == "simple"
     assert m.plan(1024, 1, 128, tile=8)["packed_bits"] == 4                          # 8 < 16 sites per 2-bit word

@@ -117,32 +117,40 @@ def test_dt_thread_engine_equals_oracle(rsos, oracle_mod, L, N, R, S, K, mcs, se
 
 
 @pytest.mark.parametrize("L,N,R,S,K,mcs,seed", [
-    (128, 1, 3, 64, 1, 6, 1),        # one tile per colour pass and realization
-    (128, 1, 9, 64, 4, 5, 21),       # C5's shape at L = 128 (K = 4); with < 32 lanes several realizations share a block
-    (256, 1, 5, 64, 4, 4, 2),        # 4 tiles per pass: 4 warps (32 lanes) .. 1 warp (8 lanes) per block
-    (512, 1, 2, 64, 4, 3, 12),       # 16 tiles per pass, 64 KiB lattice
-    (256, 2, 2, 64, 4, 4, 3),        # 4-bit sites (N = 2)
-    (512, 2, 1, 64, 4, 2, 14),       # 128 KiB lattice
+    (128, 1, 3, 64, 1, 6, 1),        # one tile per colour pass and realization: one warp per block, no cluster
+    (128, 1, 9, 64, 4, 5, 21),       # C5's shape at L = 128 (K = 4): 1024 attempts per tile and pass
+    (256, 1, 5, 64, 4, 4, 2),        # 4 tiles per pass: 4 warps in one block .. 4 blocks of one warp
+    (512, 1, 2, 64, 4, 3, 12),       # 16 tiles per pass, 256 KiB of uint8 sites: needs a cluster of >= 2 blocks
+    (256, 2, 2, 64, 4, 4, 3),        # 4-bit sites (N = 2): uint16 on chip
+    (512, 2, 1, 64, 4, 2, 14),       # 512 KiB of uint16 sites: a cluster of >= 4 blocks
     (256, 4, 1, 64, 1, 4, 4),
     (256, 7, 1, 64, 2, 3, 5),        # largest N of the 4-bit format
-    (128, 1, 2, 32, 4, 5, 6),        # S = 32, A = 256: one batch at 32 lanes
+    (128, 1, 2, 32, 4, 5, 6),        # S = 32, A = 256 attempts
     (256, 3, 2, 32, 1, 3, 16),       # S = 32, 16 tiles per pass
     (64, 2, 3, 16, 1, 5, 7),         # S = 16
-    (64, 1, 5, 16, 2, 5, 8),         # S = 16, 2-bit sites (a tile row is exactly one packed word)
+    (64, 1, 5, 16, 2, 5, 8),         # S = 16, 2-bit sites, A = 128
+    (128, 1, 2, 64, 128, 3, 11),     # A = 32: a single window per tile and pass
+    (1024, 1, 1, 64, 1, 2, 17),      # 64 tiles per pass: 8 or 16 blocks of 8 or 4 warps, rows fetched across the cluster
 ])
-@pytest.mark.parametrize("lanes", [4, 8, 16, 32])
-def test_dt_resident_engine_equals_oracle(rsos, oracle_mod, L, N, R, S, K, mcs, seed, lanes):
-    """The RESIDENT engine (packed lattice in shared memory across passes; MATCH-based hazard masks), 4 .. 32 lanes per tile."""
-    if (S * S // K) % (8 * lanes):
-        pytest.skip("a batch of 8 * lanes attempts does not divide the tile's attempts")
-    g = rsos.Rsos(L, N, R, seed, tile=S, subsweeps=K, engine=rsos.ENGINE_RESIDENT, lanes=lanes)
+@pytest.mark.parametrize("cluster", [0, 1, 2, 4, 8, 16])
+def test_dt_resident_engine_equals_oracle(rsos, oracle_mod, L, N, R, S, K, mcs, seed, cluster):
+    """The RESIDENT engine: lattice in the shared memory of a cluster of 1 .. 16 thread blocks across all passes of a
+    call, one warp per tile with 32 attempts in flight and exact conflict votes (rsos_resident.cu)."""
+    try:
+        want = rsos.plan(L, N, R, tile=S, subsweeps=K, engine=rsos.ENGINE_RESIDENT, cluster=cluster)
+    except rsos.RsosError as e:
+        assert e.code == -5
+        pytest.skip("cluster size %d does not fit this shape" % cluster)
+    g = rsos.Rsos(L, N, R, seed, tile=S, subsweeps=K, engine=rsos.ENGINE_RESIDENT, cluster=cluster)
     o = oracle_mod.Oracle(L, N, R, seed, tile=S, subsweeps=K)
     info = g.info()
-    assert info["mode"] == "DT" and info["engine"] == "resident" and info["lanes"] == lanes, info
+    assert info["mode"] == "DT" and info["engine"] == "resident" and info["cluster"] == want["cluster"], info
+    assert cluster == 0 or info["cluster"] == cluster
+    assert not info["int32_allocated"]                      # the int32 lattice exists only on demand
     for step in (1, 1, mcs - 2):                            # single MCS and several MCS inside one launch
         g.advance(step)
         o.advance(step)
-        compare(g, o, "DT resident L=%d N=%d S=%d K=%d lanes=%d t=%d" % (L, N, S, K, lanes, g.t))
+        compare(g, o, "DT resident L=%d N=%d S=%d K=%d cluster=%d t=%d" % (L, N, S, K, cluster, g.t))
     g.close()
 
 
@@ -518,9 +526,8 @@ def test_random_shapes_all_dt_engines(rsos, oracle_mod):
         first = int(rng.integers(0, 1000))
         lanes = int(rng.choice([l for l in (1, 2, 4, 8) if 8 * l <= S * S // K]))
         engines = [(rsos.ENGINE_THREAD, lanes), (rsos.ENGINE_WARP, 0)]
-        res_lanes = [l for l in (4, 8, 16, 32) if S >= 16 and L <= 8 * S and (S * S // K) % (8 * l) == 0]
-        if res_lanes:
-            engines.append((rsos.ENGINE_RESIDENT, int(rng.choice(res_lanes))))
+        if S >= 16:
+            engines.append((rsos.ENGINE_RESIDENT, 0))
         o = oracle_mod.Oracle(L, N, R, seed, tile=S, subsweeps=K, first_real=first)
         o.advance(3)
         for eng, ln in engines:
