@@ -1,24 +1,31 @@
 #!/usr/bin/env python
 """bench.py -- RSOS site-update attempts per second on B200 (BASELINE.json metric), one JSON line.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2|C4|C1|C5] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2|C4|C3/N=2|C5/L=256|...] [--impl reference]
 
 A *step* is one pass of the whole hot path over one
 batch: `mcs_per_step` Monte-Carlo steps of rsos_advance (Philox draws, origin draw, tile staging,
 attempt loop, write-back) followed by one rsos_width (int64 width reduction, result read to host).
-The default workload is BASELINE.json configs[1] (C2: L=1024, N=1, 128 realizations, DT(64,1)); its
-512 MiB of heights exceed the 126 MB L2, so no L2 flush is needed between iterations.
+The headline workload is BASELINE.json configs[1] (C2: L=1024, N=1, 128 realizations, DT(64,1)).  The
+same run then times, with the same fields under "extra", the other north_star config (C4: L=2^15, one
+surface) and short legs on C3 (N=1, 2), C5 (L=64..512) and C1, so that every BASELINE config has a
+number the driver's own run produced.  Nothing is flushed between steps: a step sweeps the same
+resident lattice 4K * mcs_per_step times exactly as a production run does; `config.l2` says what is
+resident where.
 
-value     whole-job attempts/s with the lattice resident in HBM (device-timed with CUDA events on
-          the stream the kernels run on, barrier + synchronize on both sides, max over ranks).
+value     whole-job attempts/s with the lattice resident on the device (device-timed with CUDA events
+          on the stream the kernels run on, barrier + synchronize on both sides, max over ranks).
 e2e       the same metric through the C ABI with HOST buffers: every step restores the lattice from
           a pinned host snapshot (rsos_set_state, H2D), advances it, and reads W2/<h> back (D2H).
-roofline  dominant kernel (the colour-pass update kernel): algorithmic bytes per launch
-          (8.25 B per attempt) / its average launch duration measured live by
-          rsos_kernel_time (CUDA events on the context's stream), against MEASURED_PEAKS.json.
+roofline  dominant kernel (the update kernel), bound "alu": attempts/s of the update launches alone
+          (CUDA events inside the library, rsos_kernel_time) against the rate at which the SASS-counted
+          ideal attempt loop saturates the integer alu pipe at the SM clock measured during the run
+          (DESIGN.md section 6).  `int32_equiv_sweep` keeps north_star's other candidate -- 8.25 B per
+          attempt as if the lattice were int32 -- as a labelled equivalent rate; `traffic` is the DRAM
+          bytes per launch ncu measured.
 cpu_baseline / --impl reference: the CPU oracle as it stands, on a bounded sample of the workload.
 N > 1: replicas only: rank i runs realizations [i*R, (i+1)*R), no collective
-on the data path; scaling is weak.
+on the data path; scaling is weak; the extra legs are skipped.
 """
 import argparse
 import json
@@ -46,34 +53,53 @@ def parse():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--workload", default="C2", choices=sorted(workloads.CONFIGS))
+    ap.add_argument("--workload", default="C2", help="C1..C5, or e.g. C3/N=2, C5/L=256")
     ap.add_argument("--mcs-per-step", type=int, default=0, help="MCS per step (0 = workload default)")
-    ap.add_argument("--engine", default="auto", choices=["auto", "simple", "warp", "onchip", "thread"])
+    ap.add_argument("--engine", default="auto", choices=["auto", "simple", "warp", "onchip", "thread", "resident"])
     ap.add_argument("--lanes", type=int, default=0, help="THREAD engine lanes per tile (0 = auto)")
     ap.add_argument("--tile", type=int, default=0)
     ap.add_argument("--subsweeps", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the legs on the other BASELINE configs")
+    ap.add_argument("--extra-steps", type=int, default=5, help="timed steps of each extra leg")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
 
 
+# legs of the default run besides the headline workload: the other north_star config (C4) and short legs on the rest
+EXTRA_LEGS = ("C4", "C2", "C3", "C3/N=2", "C5", "C5/L=128", "C5/L=256", "C5/L=512", "C1")
+
+
 def workload(args):
-    c = dict(workloads.CONFIGS[args.workload])
+    c = leg_config(args.workload)
     if args.tile:
         c["tile"] = args.tile
     if args.subsweeps:
         c["subsweeps"] = args.subsweeps
-    # MCS per step: about 20-40 ms of device work per step, far above launch and event overheads
-    default_mcs = {"C1": 1000, "C2": 32, "C3": 16, "C4": 4, "C5": 256}[args.workload]
-    c["mcs_per_step"] = args.mcs_per_step or default_mcs
+    if args.mcs_per_step:
+        c["mcs_per_step"] = args.mcs_per_step
     return c
+
+
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.lower().startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
 
 
 def l2_note(c, info):
     """Timing rule: say whether the inputs exceed L2 or are flushed.  A step sweeps the same resident lattice
     mcs_per_step * 4K times, exactly as a production run does, so nothing is flushed; what is resident is stated."""
     int32_mib = c["R"] * c["L"] ** 2 * 4 / 2 ** 20
+    if info and info.get("engine") == "resident":
+        return ("lattice resident in shared memory for all %d MCS of a step (packed copy in HBM %.0f MiB, touched once per "
+                "rsos_advance); nothing to flush" % (c["mcs_per_step"], int32_mib * info.get("packed_bits", 2) / 32))
     if info and info.get("engine") == "thread":
         fb = 2 if (c["N"] <= 1 and c["tile"] >= 16) else 4
         work = int32_mib * fb / 32
@@ -85,23 +111,29 @@ def l2_note(c, info):
 
 
 def traffic_note(workload_name, info):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full summary (profiles/traffic.csv), or None."""
+    """(DRAM bytes per launch of the dominant kernel, where it comes from) from the committed ncu --set full
+    summaries (profiles/traffic.csv: key, bytes, commit the capture was taken at, capture file), or (None, None)."""
     key = "%s/%s/lanes%d" % (workload_name, info["engine"], info.get("lanes", 0))
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.csv")) as f:
             for line in f:
                 parts = line.strip().split(",")
-                if len(parts) == 2 and parts[0] == key:
-                    return float(parts[1])
+                if len(parts) >= 2 and parts[0] == key:
+                    src = "profiles/traffic.csv" + (" (captured at commit %s, %s)" % (parts[2], parts[3]) if len(parts) >= 4 else "")
+                    return float(parts[1]), src
     except (OSError, ValueError):
         pass
-    return None
+    return None, None
 
 
 def config_dict(args, c, n_gpus, info=None):
+    return config_dict_for(args.workload, c, n_gpus, info)
+
+
+def config_dict_for(name, c, n_gpus, info=None):
     mode = "RS" if 2 * c["tile"] > c["L"] else "DT(%d,%d)" % (c["tile"], c["subsweeps"])
     return {"workload": "%s: RSOS N=%d, L=%d periodic, %d realizations per GPU, int32 heights, flat start, seed %d"
-                        % (args.workload, c["N"], c["L"], c["R"], c["seed"]),
+                        % (name, c["N"], c["L"], c["R"], c["seed"]),
             "schedule": mode, "mcs_per_step": c["mcs_per_step"],
             "step": "rsos_advance(mcs_per_step) + rsos_width",
             "l2": l2_note(c, info),
@@ -212,7 +244,8 @@ def run_reference(args):
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
             "config": config_dict(args, c, args.gpus),
-            "cpu_baseline": {"value": v / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "cpu_baseline": {"value": v / 1e9, "unit": UNIT, "cores": cores, "cpu_model": cpu_model(), "kind": "oracle",
+                             "sample": desc},
             "e2e": {"value": v / 1e9, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -221,8 +254,142 @@ def run_reference(args):
 # ---------------------------------------------------------------------------------------------
 # The B200 arm
 # ---------------------------------------------------------------------------------------------
-def run_b200(args):
+# Instruction roofline.  SASS count of the one-lane-per-tile attempt loop of
+# thread_dt_kernel<6, 2, 1> (profiles/r2_sass_attempt_loop.md): per attempt, Philox included,
+IDEAL_LOOP = {"thread_instr": 47.875, "alu_pipe": 26.125, "fma_pipe": 15.5, "lsu": 6.0, "other": 0.25}
+SURVEY_FLOOR_INSTR = 22.0     # SURVEY 8(d)'s hand estimate, kept for comparison
+
+
+def alu_peak_attempts_per_s(sm_count, sm_mhz):
+    """Attempts/s at which the ideal loop saturates an SM sub-partition: one warp instruction issued per cycle,
+    the integer alu pipe and the fma pipe each take one warp instruction per two cycles (B300_MICROARCH.md,
+    'fma vs alu split', rt_SMSP = 2).  The slowest of the three binds (the alu pipe: 52.25 cycles per 32 attempts)."""
+    cyc = max(IDEAL_LOOP["thread_instr"], 2.0 * IDEAL_LOOP["alu_pipe"], 2.0 * IDEAL_LOOP["fma_pipe"])
+    return sm_count * 4 * 32 / cyc * sm_mhz * 1e6
+
+
+def leg_config(name):
+    """name = C1..C5, 'C3/N=2', 'C5/L=256' ... -> workload dict (utils/workloads.py holds the numbers)."""
+    base, _, mod = name.partition("/")
+    c = dict(workloads.CONFIGS[base])
+    if mod:
+        k, v = mod.split("=")
+        c[k] = int(v)
+        if base == "C5" and k == "L":
+            c["R"] = workloads.c5_realizations(c["L"])
+            c["mcs"] = workloads.c5_mcs(c["L"])
+    # MCS per step: 10-40 ms of device work per step, far above launch and event overheads
+    dflt = {"C1": 1000, "C2": 32, "C3": 16, "C4": 4, "C5": 256}[base]
+    if base == "C5" and c["L"] > 64:
+        dflt = {128: 256, 256: 256, 512: 128}[c["L"]]
+    c["mcs_per_step"] = dflt
+    return c
+
+
+def run_leg(pkg, torch, name, c, steps, warmup, engine, lanes, rank, world, local, barrier, do_e2e, dist):
+    """One timed leg: `warmup` untimed steps, then exactly `steps` steps between CUDA events on the kernels' stream
+    (barrier + synchronize on both sides, max over ranks), clocks sampled during the timed region."""
     import numpy as np
+    L, N, R, mcs = c["L"], c["N"], c["R"], c["mcs_per_step"]
+    stream = torch.cuda.Stream()
+    first_real, _ = workloads.replica_range(rank, world, R)
+    g = pkg.Rsos(L, N, R, c["seed"], tile=c["tile"], subsweeps=c["subsweeps"], first_real=first_real, engine=engine,
+                 stream=stream.cuda_stream, lanes=lanes)
+    info = g.info()
+    att_step = workloads.attempts(L, R, mcs)
+
+    def step():
+        g.advance(mcs)
+        return g.width()
+
+    for _ in range(max(3, warmup)):
+        step()
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    if sampler:
+        sampler.start()
+        time.sleep(0.3)                                    # let nvidia-smi come up before the timed region
+    g.kernel_time(True)                                    # per-advance CUDA events inside the library
+    launches0 = g.info()["launches"]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    if sampler:
+        sampler.mark()
+    e0.record(stream)
+    for _ in range(steps):
+        W2, hmean = step()
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop() if sampler else None
+    upd_ms, upd_launches = g.kernel_time(False)
+    launches = g.info()["launches"] - launches0
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    value = att_step * steps * world / (ms * 1e-3)
+
+    # ---- e2e: host buffers through the C ABI, H2D + D2H inside the timed region -----------------
+    e2e = None
+    if do_e2e:
+        snap = torch.empty((R, L, L), dtype=torch.int32, pin_memory=True)
+        snap_np = snap.numpy()
+        g.heights(out=snap_np)
+        t_snap = g.t
+        _, _, acc = g.sums()
+        for _ in range(2):
+            g.set_state(snap_np, t_snap, acc)
+            step()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            g.set_state(snap_np, t_snap, acc)              # H2D: R*L*L int32 + R int64
+            step()                                         # advance + width (D2H: sums, accepted)
+        barrier()
+        dt = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": att_step * steps * world / dt / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": R * L * L * 4 + R * 8, "d2h_bytes_per_step": R * 5 * 8 + 4,
+               "what": "rsos_set_state(pinned host snapshot) + rsos_advance + rsos_width per step, wall clock"}
+        del snap
+
+    # ---- roofline of the dominant kernel (the update kernel) ------------------------------------
+    hbm, how = peaks()
+    n_l = max(1, upd_launches)
+    per_launch_att = att_step * steps / n_l
+    avg_ms = upd_ms / n_l
+    kernel_rate = att_step * steps / (upd_ms * 1e-3)       # attempts/s of the update kernels alone
+    sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
+    peak = alu_peak_attempts_per_s(info["sm_count"], sm_mhz)
+    traffic, traffic_src = traffic_note(name, info)
+    sweep_gbs = kernel_rate * BYTES_PER_ATTEMPT * c["subsweeps"] / 1e9 if info["mode"] == "DT" else None
+    roofline = {"bound": "alu", "achieved": kernel_rate / 1e9, "peak": peak / 1e9, "unit": "G attempts/s",
+                "frac": kernel_rate / peak, "traffic": traffic, "traffic_source": traffic_src,
+                "peak_source": "derived (DESIGN.md section 6): %d SMs x 4 schedulers x 32 lanes / 52.25 cycles per 32 attempts "
+                               "(alu pipe of the SASS-counted ideal loop, profiles/r2_sass_attempt_loop.md) x %.0f MHz measured"
+                               % (info["sm_count"], sm_mhz),
+                "kernel": "update kernel, engine=%s" % info["engine"],
+                "attempts_per_launch": per_launch_att, "avg_launch_ms": avg_ms, "update_launches": int(upd_launches),
+                "update_share_of_step": upd_ms / ms,
+                "frac_of_survey_floor_22_instr": kernel_rate / (info["sm_count"] * 4 * 32 * sm_mhz * 1e6 / SURVEY_FLOOR_INSTR),
+                # north_star's other candidate, kept as a labelled int32-EQUIVALENT sweep rate: the packed working
+                # lattice moves far fewer bytes (see traffic), so this is not what binds
+                "int32_equiv_sweep": {"bytes_per_attempt": BYTES_PER_ATTEMPT * c["subsweeps"], "GBps": sweep_gbs,
+                                      "hbm_peak_GBps": hbm, "peak_source": how,
+                                      "frac": (sweep_gbs / hbm) if sweep_gbs else None}}
+    out = {"workload": name, "value": value / 1e9, "unit": UNIT, "steps": steps, "warmup": max(3, warmup),
+           "ms_per_step": ms / steps, "config": None, "engine": info, "clocks": clocks, "e2e": e2e,
+           "gpu_launches": int(launches), "roofline": roofline,
+           "result_check": {"W2_mean": float(np.mean(W2)), "hmean_mean": float(np.mean(hmean)), "t_mcs": int(g.t)}}
+    g.close()
+    return out
+
+
+def run_b200(args):
     import torch
     import torch.distributed as dist
     if not torch.cuda.is_available():
@@ -246,110 +413,37 @@ def run_b200(args):
     import paper_1605_02620_b200 as pkg
 
     c = workload(args)
-    L, N, R, mcs = c["L"], c["N"], c["R"], c["mcs_per_step"]
-    engine = {"auto": 0, "simple": 1, "warp": 2, "onchip": 3, "thread": 4}[args.engine]
-    stream = torch.cuda.Stream()
-    heights = torch.empty((R, L, L), dtype=torch.int32, device="cuda")      # device memory only: plumbing
-    first_real, _ = workloads.replica_range(rank, world, R)
-    g = pkg.Rsos(L, N, R, c["seed"], tile=c["tile"], subsweeps=c["subsweeps"], first_real=first_real, engine=engine,
-                 d_heights=heights.data_ptr(), stream=stream.cuda_stream, lanes=args.lanes)
-    info = g.info()
-    att_step = workloads.attempts(L, R, mcs)
+    engine = {"auto": 0, "simple": 1, "warp": 2, "onchip": 3, "thread": 4, "resident": 5}[args.engine]
+    head = run_leg(pkg, torch, args.workload, c, args.steps, args.warmup, engine, args.lanes, rank, world, local, barrier,
+                   not args.no_e2e, dist)
 
-    def step():
-        g.advance(mcs)
-        return g.width()
-
-    for _ in range(max(3, args.warmup)):
-        step()
-    barrier()
-
-    # ---- timed region: exactly K steps, CUDA events on the kernels' stream ----------------------
-    sampler = ClockSampler(local) if rank == 0 else None
-    if sampler:
-        sampler.start()
-        time.sleep(0.3)                                    # let nvidia-smi come up before the timed region
-    g.kernel_time(True)                                    # per-advance CUDA events inside the library
-    launches0 = g.info()["launches"]
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    if sampler:
-        sampler.mark()
-    e0.record(stream)
-    for _ in range(args.steps):
-        W2, hmean = step()
-    e1.record(stream)
-    barrier()
-    ms = e0.elapsed_time(e1)
-    clocks = sampler.stop() if sampler else None
-    upd_ms, upd_launches = g.kernel_time(False)
-    launches = g.info()["launches"] - launches0
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = att_step * args.steps * world / (ms * 1e-3)
-
-    # ---- e2e: host buffers through the C ABI, H2D + D2H inside the timed region -----------------
-    e2e = None
-    if not args.no_e2e:
-        snap = torch.empty((R, L, L), dtype=torch.int32, pin_memory=True)
-        snap_np = snap.numpy()
-        g.heights(out=snap_np)
-        t_snap = g.t
-        _, _, acc = g.sums()
-        for _ in range(2):
-            g.set_state(snap_np, t_snap, acc)
-            step()
-        barrier()
-        t0 = time.perf_counter()
-        for _ in range(args.steps):
-            g.set_state(snap_np, t_snap, acc)              # H2D: R*L*L int32 + R int64
-            step()                                         # advance + width (D2H: sums, accepted)
-        barrier()
-        dt = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([dt], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
-        e2e = {"value": att_step * args.steps * world / dt / 1e9, "unit": UNIT,
-               "h2d_bytes_per_step": R * L * L * 4 + R * 8, "d2h_bytes_per_step": R * 5 * 8 + 4,
-               "what": "rsos_set_state(pinned host snapshot) + rsos_advance + rsos_width per step, wall clock"}
-        del snap
+    # ---- the other BASELINE configs, same fields, fewer steps (one GPU only) -------------------------
+    extra = {}
+    if world == 1 and not args.no_extra:
+        for name in EXTRA_LEGS:
+            if name == args.workload:
+                continue
+            ce = leg_config(name)
+            leg = run_leg(pkg, torch, name, ce, args.extra_steps, 3, 0, 0, rank, world, local, barrier,
+                          not args.no_e2e and name in ("C4",), dist)
+            leg["config"] = config_dict_for(name, ce, 1, leg["engine"])
+            extra[name] = leg
 
     if rank != 0:
-        g.close()
         if world > 1:
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (the update kernel) ------------------------------------
-    hbm, how = peaks()
-    per_launch_att = att_step * args.steps / max(1, upd_launches)
-    avg_ms = upd_ms / max(1, upd_launches)
-    achieved = per_launch_att * BYTES_PER_ATTEMPT / (avg_ms * 1e-3) / 1e9
-    sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
-    # issue bound = SMs x 4 schedulers x 32 lanes x measured SM clock / 22 instructions per attempt
-    alu_bound = info["sm_count"] * 4 * 32 * sm_mhz * 1e6 / 22.0
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": hbm, "unit": "GB/s", "frac": achieved / hbm,
-                "traffic": traffic_note(args.workload, info), "peak_source": how, "kernel": "update kernel, engine=%s" % info["engine"],
-                "bytes_per_attempt": BYTES_PER_ATTEMPT, "attempts_per_launch": per_launch_att,
-                "avg_launch_ms": avg_ms, "update_share_of_step": upd_ms / ms,
-                "alu_bound_attempts_per_s": alu_bound, "frac_of_alu_bound": (att_step * args.steps / (upd_ms * 1e-3)) / alu_bound,
-                "hbm_bound_attempts_per_s": hbm * 1e9 / BYTES_PER_ATTEMPT}
-
     cpu = None
     if not args.no_cpu_baseline and world == 1:
         v, cores, desc, _ = oracle_sample(c, args.cpu_seconds)
-        cpu = {"value": v / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+        cpu = {"value": v / 1e9, "unit": UNIT, "cores": cores, "cpu_model": cpu_model(), "kind": "oracle", "sample": desc}
 
-    line = {"metric": METRIC, "value": value / 1e9, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "int32", "data": "synthetic", "config": config_dict(args, c, world, info),
-            "engine": info, "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
-            "cpu_baseline": cpu, "result_check": {"W2_mean": float(np.mean(W2)), "hmean_mean": float(np.mean(hmean)),
-                                                  "t_mcs": int(g.t)}}
-    g.close()
+    line = {"metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(3, args.warmup), "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int32", "data": "synthetic", "config": config_dict(args, c, world, head["engine"]),
+            "engine": head["engine"], "clocks": head["clocks"], "e2e": head["e2e"], "gpu_launches": head["gpu_launches"],
+            "roofline": head["roofline"], "cpu_baseline": cpu, "result_check": head["result_check"], "extra": extra}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
