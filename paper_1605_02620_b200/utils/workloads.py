@@ -31,6 +31,21 @@ def log_spaced_times(t_max, n=64):
     return sorted({int(round(t_max ** (j / (n - 1)))) for j in range(n)})
 
 
+def eq10_times(t_max, m=0.01, t0=0.0):
+    """The paper's measurement schedule, Eq. (10): t_{i+1} = (t_i + 10) e^m with m = 0.01, t_0 = 0.
+    The recursion gives real numbers and the paper does not say how they are rounded (reading Q11): each t_i is
+    rounded to the nearest integer MCS, duplicates are dropped, times beyond t_max are cut."""
+    out, t = [], float(t0)
+    while True:
+        t = (t + 10.0) * math.exp(m)
+        ti = int(round(t))
+        if ti > t_max:
+            break
+        if not out or ti > out[-1]:
+            out.append(ti)
+    return out
+
+
 def attempts(L, R, mcs):
     """1 MCS = L*L attempts per realization (reading Q4)."""
     return int(L) * int(L) * int(R) * int(mcs)
