@@ -20,6 +20,9 @@
  *   - domain decomposition by double tiling with an origin moved randomly after each
  *     sweep; independent realizations.
  * What the paper leaves open (tile size, colour order, RNG, slot layout) is fixed by S8c.1.
+ * Lattice sides that are not powers of two (the paper's L = 9605; irregular tilings)
+ * follow the general-L schedule DTG / RSG of DESIGN.md section 2b: tiles of two sizes that divide
+ * the lattice, sites drawn by an exactly uniform bounded draw (multiply-shift with rejection).
  *
  * Pins (tests/test_oracle_*.py, all CPU): Eq. (6) invariant after every attempt, monotone
  * heights, sum h == accepted, random-deposition closed form, exact Markov-chain enumeration
@@ -108,8 +111,9 @@ typedef struct rsos_oracle {
     uint32_t L, R, S, K, first_real;
     int64_t  N;
     uint64_t seed, t;
-    int      mode_dt;        /* 1 = DT(S,K), 0 = RS (2S > L, or L not a power of two)        */
+    int      mode_dt;        /* 1 = DT(S,K) (DTG when L is not a power of two), 0 = RS (2S > L) */
     int      pow2;           /* L is a power of two                                          */
+    uint32_t T;              /* general-L DT mode: tiles per side (even); 0 otherwise        */
     uint32_t lgL, lgS;
     int32_t *h;              /* R * L * L                                                    */
     int64_t *accepted;       /* R                                                            */
@@ -128,8 +132,8 @@ const char *rsos_oracle_last_error(void) { return g_err; }
 
 /* ------------------------------------------------------------------------------------------
  * Create / free.  S8c.1 steps 1 and 3.  S = tile side, K = sub-sweeps per MCS.
- *   mode RS  when 2*S > L (or L is not a power of two: test-only general-L draw, see below);
- *   mode DT  otherwise; needs S, K powers of two, K | S*S, S*S/K >= 32.
+ *   mode RS  when 2*S > L;  mode DT  otherwise; needs S, K powers of two, K | S*S, S*S/K >= 32.
+ *   L not a power of two: the general-L forms RSG / DTG of the same two modes (D:2b).
  * All heights 0, accepted 0, t = 0 (flat start).
  * ------------------------------------------------------------------------------------------ */
 rsos_oracle *rsos_oracle_create(uint32_t L, int64_t N, uint32_t R, uint64_t seed,
@@ -144,8 +148,13 @@ rsos_oracle *rsos_oracle_create(uint32_t L, int64_t N, uint32_t R, uint64_t seed
     c->L = L; c->N = N; c->R = R; c->seed = seed; c->first_real = first_real;
     c->pow2 = is_pow2(L);
     c->lgL = ilog2(L);
-    if (!c->pow2 || 2 * (uint64_t)S > L) {          /* RS: one tile = the whole lattice */
+    if (2 * (uint64_t)S > L) {                      /* RS: one tile = the whole lattice */
         c->mode_dt = 0; c->S = L; c->K = 1; c->lgS = c->lgL;
+    } else if (!c->pow2) {                          /* DTG: D:2b, T = 2 floor(L / 2S) tiles per side */
+        if (!is_pow2(S) || S < 8 || !is_pow2(K) || ((uint64_t)S * S) % K || (uint64_t)S * S / K < 32) {
+            snprintf(g_err, sizeof g_err, "bad S/K"); free(c); return NULL;
+        }
+        c->mode_dt = 1; c->S = S; c->K = K; c->lgS = ilog2(S); c->T = 2 * (L / (2 * S));
     } else {
         if (!is_pow2(S) || S < 8 || !is_pow2(K) || ((uint64_t)S * S) % K || (uint64_t)S * S / K < 32) {
             snprintf(g_err, sizeof g_err, "bad S/K"); free(c); return NULL;
@@ -197,8 +206,7 @@ static int attempt_checked(rsos_oracle *c, int32_t *h, uint32_t x, uint32_t y)
  *   o = Philox(counter = (q, tile id, u, r), key = seed);
  *   v = 16-bit slot j of o (low half first) or o[j];  dx = v & (Se-1), dy = (v >> lg Se) & (Se-1);
  *   site x = (ox + I*S + dx) & (L-1), y = (oy + J*S + dy) & (L-1).
- * General-L draw (L not a power of two; RS only; used by the 3x3 pin): w = 32 and
- *   site = ((uint64)v * L*L) >> 32, x = site % L, y = site / L.
+ * (Lattice sides that are not powers of two never come here: run_tile_general.)
  * Returns the number of accepted deposits.
  * ------------------------------------------------------------------------------------------ */
 static int64_t run_tile(rsos_oracle *c, int32_t *h, uint32_t rg, uint32_t u, uint32_t tile_id,
@@ -206,7 +214,7 @@ static int64_t run_tile(rsos_oracle *c, int32_t *h, uint32_t rg, uint32_t u, uin
 {
     const uint32_t L = c->L;
     const uint32_t key[2] = { (uint32_t)(c->seed & 0xffffffffu), (uint32_t)(c->seed >> 32) };
-    const uint32_t w = (c->pow2 && 2 * lgSe <= 16) ? 16 : 32;
+    const uint32_t w = (2 * lgSe <= 16) ? 16 : 32;
     const uint32_t ns = 128 / w;
     int64_t acc = 0;
     uint64_t a = 0;
@@ -215,19 +223,143 @@ static int64_t run_tile(rsos_oracle *c, int32_t *h, uint32_t rg, uint32_t u, uin
         rsos_oracle_philox(ctr, key, o);
         for (uint32_t j = 0; j < ns && a < A; ++j, ++a) {
             uint32_t v = (w == 16) ? (o[j >> 1] >> (16 * (j & 1))) & 0xffffu : o[j];
-            uint32_t x, y;
-            if (c->pow2) {
-                uint32_t dx = v & (Se - 1), dy = (v >> lgSe) & (Se - 1);
-                x = (x0 + dx) & (L - 1);
-                y = (y0 + dy) & (L - 1);
-            } else {
-                uint32_t site = (uint32_t)(((uint64_t)v * ((uint64_t)L * L)) >> 32);
-                x = site % L; y = site / L;
-            }
+            uint32_t dx = v & (Se - 1), dy = (v >> lgSe) & (Se - 1);
+            uint32_t x = (x0 + dx) & (L - 1);
+            uint32_t y = (y0 + dy) & (L - 1);
             acc += attempt_checked(c, h, x, y);
         }
     }
     return acc;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * General-L schedule, for lattice sides that are not powers of two.
+ *
+ * Word stream of (tile id, u, r): word i = o[i & 3] of Philox(counter (i >> 2, tile id, u, r)).
+ * draw(n), exactly uniform on [0, n) (Lemire's multiply-shift with rejection in its plain form):
+ *     thr = 2^32 mod n;  repeat  v = next word;  m = v * n (64 bit)  until (m mod 2^32) >= thr;
+ *     return m >> 32.
+ * Every value of [0, n) is hit by exactly floor(2^32 / n) of the 2^32 words (pinned by a census
+ * over all words, tests/test_oracle_general.py); a rejected word (probability < n / 2^32) is
+ * skipped and the next word of the stream is taken.
+ * ------------------------------------------------------------------------------------------ */
+typedef struct { uint32_t ctr[4], key[2], o[4]; uint32_t j; } word_stream;
+
+static void stream_init(word_stream *s, const rsos_oracle *c, uint32_t tile_id, uint32_t u, uint32_t rg)
+{
+    s->ctr[0] = 0; s->ctr[1] = tile_id; s->ctr[2] = u; s->ctr[3] = rg;
+    s->key[0] = (uint32_t)(c->seed & 0xffffffffu); s->key[1] = (uint32_t)(c->seed >> 32);
+    s->j = 4;                                   /* nothing generated yet */
+}
+
+static uint32_t stream_next(word_stream *s)
+{
+    if (s->j == 4) { rsos_oracle_philox(s->ctr, s->key, s->o); s->ctr[0] += 1; s->j = 0; }
+    return s->o[s->j++];
+}
+
+uint32_t rsos_oracle_bounded(uint32_t v, uint32_t n, int *accepted)
+{
+    const uint32_t thr = (uint32_t)(0x100000000ull % n);
+    const uint64_t m = (uint64_t)v * n;
+    *accepted = (uint32_t)m >= thr;
+    return (uint32_t)(m >> 32);
+}
+
+static uint32_t stream_draw(word_stream *s, uint32_t n)
+{
+    for (;;) {
+        int ok;
+        const uint32_t r = rsos_oracle_bounded(stream_next(s), n, &ok);
+        if (ok) return r;
+    }
+}
+
+/* Census of draw(n) over ALL 2^32 words (test hook): counts[v] = words mapped to v, *rejected = words
+ * rejected.  Exact uniformity means counts[v] == floor(2^32 / n) for every v and *rejected == 2^32 mod n. */
+void rsos_oracle_bounded_census(uint32_t n, uint64_t *counts, uint64_t *rejected)
+{
+    uint64_t rej = 0;
+    for (uint32_t v = 0; v < n; ++v) counts[v] = 0;
+#ifdef _OPENMP
+#pragma omp parallel
+#endif
+    {
+        uint64_t *loc = (uint64_t *)calloc(n, sizeof(uint64_t));
+        uint64_t lrej = 0;
+#ifdef _OPENMP
+#pragma omp for schedule(static)
+#endif
+        for (int64_t w = 0; w < 0x100000000ll; ++w) {
+            int ok;
+            const uint32_t r = rsos_oracle_bounded((uint32_t)w, n, &ok);
+            if (ok) loc[r] += 1; else lrej += 1;
+        }
+#ifdef _OPENMP
+#pragma omp critical
+#endif
+        { for (uint32_t v = 0; v < n; ++v) counts[v] += loc[v]; rej += lrej; }
+        free(loc);
+    }
+    *rejected = rej;
+}
+
+/* Boundary of tile column / row i of T on a lattice of side L: floor(i * L / T)  (D:2b). */
+static uint32_t tile_edge(uint32_t i, uint32_t L, uint32_t T) { return (uint32_t)(((uint64_t)i * L) / T); }
+
+/* All A attempts of one general tile of w x hgt sites whose first site is (x0, y0), in order:
+ *   s = draw(w * hgt);  dx = s mod w, dy = s div w;  site ((x0 + dx) mod L, (y0 + dy) mod L).   D:2b. */
+static int64_t run_tile_general(rsos_oracle *c, int32_t *h, uint32_t rg, uint32_t u, uint32_t tile_id,
+                                uint32_t x0, uint32_t y0, uint32_t w, uint32_t hgt, uint64_t A)
+{
+    const uint32_t L = c->L;
+    word_stream st;
+    stream_init(&st, c, tile_id, u, rg);
+    int64_t acc = 0;
+    for (uint64_t a = 0; a < A; ++a) {
+        const uint32_t s = stream_draw(&st, w * hgt);
+        const uint32_t dx = s % w, dy = s / w;
+        acc += attempt_checked(c, h, (x0 + dx) % L, (y0 + dy) % L);
+    }
+    return acc;
+}
+
+/* One MCS of the general-L schedule (D:2b).  RSG: one tile = the lattice, origin (0, 0), L*L attempts.
+ * DTG: T = 2 floor(L / 2S) tiles per side with edges floor(i L / T); for k < K: u = t K + k; origin
+ * (ox, oy) = (draw(L), draw(L)) from the stream of tile id 0xFFFFFFFF; colours 0..3 as in DT; tile
+ * (I, J) of n = w * hgt sites makes floor((k+1) n / K) - floor(k n / K) attempts in sub-sweep k (n per MCS). */
+static void one_mcs_general(rsos_oracle *c, uint32_t rl, uint64_t t, int par_tiles)
+{
+    const uint32_t L = c->L, K = c->K, T = c->T;
+    int32_t *h = c->h + (size_t)rl * L * L;
+    const uint32_t rg = c->first_real + rl;
+    if (!c->mode_dt) {
+        c->accepted[rl] += run_tile_general(c, h, rg, (uint32_t)t, 0, 0, 0, L, L, (uint64_t)L * L);
+        return;
+    }
+    const uint32_t half = T / 2, ntile = half * half;
+    for (uint32_t k = 0; k < K; ++k) {
+        const uint32_t u = (uint32_t)(t * K + k);
+        word_stream os;
+        stream_init(&os, c, 0xFFFFFFFFu, u, rg);
+        const uint32_t ox = stream_draw(&os, L);
+        const uint32_t oy = stream_draw(&os, L);
+        for (uint32_t p = 0; p < 4; ++p) {
+            int64_t acc = 0;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(dynamic, 4) reduction(+:acc) if (par_tiles)
+#endif
+            for (uint32_t n = 0; n < ntile; ++n) {
+                const uint32_t I = 2 * (n % half) + (p & 1), J = 2 * (n / half) + (p >> 1);
+                const uint32_t bx = tile_edge(I, L, T), by = tile_edge(J, L, T);
+                const uint32_t w = tile_edge(I + 1, L, T) - bx, hgt = tile_edge(J + 1, L, T) - by;
+                const uint64_t sites = (uint64_t)w * hgt;
+                const uint64_t A = ((uint64_t)(k + 1) * sites) / K - ((uint64_t)k * sites) / K;
+                acc += run_tile_general(c, h, rg, u, J * T + I, (ox + bx) % L, (oy + by) % L, w, hgt, A);
+            }
+            c->accepted[rl] += acc;
+        }
+    }
 }
 
 static uint64_t splitmix64(uint64_t *s)
@@ -246,6 +378,7 @@ static void one_mcs(rsos_oracle *c, uint32_t rl, uint64_t t, int par_tiles)
     const uint32_t L = c->L, S = c->S, K = c->K;
     int32_t *h = c->h + (size_t)rl * L * L;
     const uint32_t rg = c->first_real + rl;
+    if (!c->pow2) { one_mcs_general(c, rl, t, par_tiles); return; }
     if (!c->mode_dt) {
         c->accepted[rl] += run_tile(c, h, rg, (uint32_t)t, 0, 0, 0, L, c->lgL, (uint64_t)L * L);
         return;

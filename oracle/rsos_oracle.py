@@ -69,8 +69,27 @@ def lib():
         l.rsos_oracle_height_moments.restype = C.c_int
         l.rsos_oracle_power_sums.argtypes = [vp, u32, i64, C.POINTER(u64)]
         l.rsos_oracle_power_sums.restype = C.c_int
+        l.rsos_oracle_bounded.argtypes = [u32, u32, C.POINTER(C.c_int)]
+        l.rsos_oracle_bounded.restype = u32
+        l.rsos_oracle_bounded_census.argtypes = [u32, vp, C.POINTER(u64)]
+        l.rsos_oracle_bounded_census.restype = None
         _lib = l
     return _lib
+
+
+def bounded(v, n):
+    """One step of the exactly uniform bounded draw: (value in [0, n), accepted?)."""
+    ok = C.c_int()
+    r = lib().rsos_oracle_bounded(int(v) & 0xFFFFFFFF, int(n), C.byref(ok))
+    return int(r), bool(ok.value)
+
+
+def bounded_census(n):
+    """(counts[n], rejected) of the bounded draw over all 2^32 words (a few seconds)."""
+    counts = np.zeros(int(n), dtype=np.uint64)
+    rej = C.c_uint64()
+    lib().rsos_oracle_bounded_census(int(n), counts.ctypes.data, C.byref(rej))
+    return counts, int(rej.value)
 
 
 def philox(ctr, key):
