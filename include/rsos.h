@@ -53,7 +53,8 @@ enum {
                              /* at least RSOS_THREAD_MIN_TILES active tiles, else RESIDENT when   */
                              /* it applies, else WARP, else SIMPLE                                */
     RSOS_ENGINE_SIMPLE = 1,  /* one thread per active tile, heights in global memory (slow;       */
-                             /* the literal loop nest of D:2, kept as an on-device cross-check)   */
+                             /* the literal loop nest of D:2, kept as an on-device cross-check;   */
+                             /* also the engine of the general-L schedule D:2b)                   */
     RSOS_ENGINE_WARP   = 2,  /* DT mode: one warp per active tile, (S+2)^2 window staged in       */
                              /* shared memory, 32 attempts in flight with exact conflict votes;   */
                              /* needs tile <= 128 and N <= 31                                     */
@@ -98,13 +99,17 @@ typedef struct rsos_opts {
 /*
  * rsos_init -- create a context: R flat surfaces h = 0 at t = 0, accepted = 0.
  *   ctx   out, host: receives the context (NULL on failure)
- *   L     lattice side, power of two, 4 <= L <= 65536 (periodic in both directions, reading Q2)
+ *   L     lattice side, 4 <= L <= 65536 (periodic in both directions, reading Q2).  Powers of two run the
+ *         schedule D:2 on every engine; any other L (the paper's L = 9605) runs the general-L schedule
+ *         D:2b -- tiles of two sizes that divide the lattice, sites drawn by an exactly uniform bounded
+ *         draw -- on the SIMPLE engine only (int32 heights in global memory)
  *   N     height-difference bound of Eq. (6), 1 <= N <= 127
  *   R     number of independent realizations, >= 1, R*L*L*4 bytes must fit on the device
  *   seed  Philox key (low word, high word)
  *   opts  host, may be NULL
  * Errors: RSOS_EINVAL (L, N, R, tile, subsweeps, engine, misaligned d_heights), RSOS_EUNSUP
- * (engine cannot run the mode), RSOS_ENOMEM, RSOS_ECUDA.
+ * (engine cannot run the mode, or an engine other than AUTO / SIMPLE with L not a power of two),
+ * RSOS_ENOMEM, RSOS_ECUDA.
  */
 int rsos_init(rsos_ctx **ctx, uint32_t L, uint32_t N, uint32_t R, uint64_t seed, const rsos_opts *opts);
 

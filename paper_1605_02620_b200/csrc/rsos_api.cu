@@ -104,8 +104,8 @@ static void destroy(rsos_ctx *c)
 // Host-only planning: argument checks, mode, engine selection, lanes and packed-site width.
 // Shared by rsos_init and rsos_plan; needs no device.
 struct Plan {
-    bool mode_dt;
-    uint32_t engine, S, K, lanes, field_bits, cluster;
+    bool mode_dt, general;
+    uint32_t engine, S, K, lanes, field_bits, cluster, T;
     uint64_t pass_tiles;
 };
 
@@ -113,7 +113,8 @@ constexpr size_t SMEM_LIMIT_SM100 = 227u * 1024u;        // opt-in shared memory
 
 static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, int sm_count, size_t smem_limit, Plan *pl)
 {
-    if (!is_pow2(L) || L < 4 || L > 65536) return fail(RSOS_EINVAL, "L = %u must be a power of two in [4, 65536]", L);
+    if (L < 4 || L > 65536) return fail(RSOS_EINVAL, "L = %u must be in [4, 65536]", L);
+    const bool general = !is_pow2(L);                      // general-L schedule RSG / DTG (D:2b)
     if (N < 1 || N > 127) return fail(RSOS_EINVAL, "N = %u must be in [1, 127]", N);
     if (R < 1) return fail(RSOS_EINVAL, "R must be >= 1");
     if (opt.lanes != 0 && opt.lanes != 1 && opt.lanes != 2 && opt.lanes != 4 && opt.lanes != 8)
@@ -136,14 +137,15 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
 
     // engine selection (include/rsos.h)
     uint32_t engine = opt.engine;
-    const bool warp_ok = mode_dt && S <= 128 && N <= 31;
-    const bool thread_ok = mode_dt && S <= 64 && N <= 7;
-    const bool onchip_ok = !mode_dt && L <= 128 && N <= 31;
-    const uint64_t pass_tiles = mode_dt ? (uint64_t)R * (L / S / 2) * (L / S / 2) : 0;
+    const bool warp_ok = !general && mode_dt && S <= 128 && N <= 31;
+    const bool thread_ok = !general && mode_dt && S <= 64 && N <= 7;
+    const bool onchip_ok = !general && !mode_dt && L <= 128 && N <= 31;
+    const uint32_t T = !mode_dt ? 0u : general ? 2u * (L / (2u * S)) : L / S;
+    const uint64_t pass_tiles = mode_dt ? (uint64_t)R * (T / 2) * (T / 2) : 0;
     // RESIDENT: blocks per cluster (= per realization) = opts.cluster, else chosen from the shared memory a block
     // may use and the number of blocks the machine needs (rsos_resident.cu)
     uint32_t res_cluster = 0;
-    if (mode_dt) {
+    if (mode_dt && !general) {
         if (opt.cluster) { if (resident_ok(L, N, S, K, opt.cluster, smem_limit)) res_cluster = opt.cluster; }
         else res_cluster = resident_cluster_size(L, N, S, K, R, sm_count, smem_limit);
     }
@@ -162,7 +164,10 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
         return fail(RSOS_EUNSUP, "engine THREAD needs DT mode (2*tile <= L), tile <= 64 and N <= 7");
     if (engine == RSOS_ENGINE_ONCHIP && !onchip_ok)
         return fail(RSOS_EUNSUP, "engine ONCHIP needs RS mode (2*tile > L), L <= 128 and N <= 31");
-    pl->mode_dt = mode_dt; pl->engine = engine; pl->S = S; pl->K = K; pl->pass_tiles = pass_tiles;
+    if (general && engine != RSOS_ENGINE_SIMPLE)
+        return fail(RSOS_EUNSUP, "L = %u is not a power of two: only the SIMPLE engine runs the general-L schedule", L);
+    pl->mode_dt = mode_dt; pl->general = general; pl->T = T;
+    pl->engine = engine; pl->S = S; pl->K = K; pl->pass_tiles = pass_tiles;
     pl->lanes = 0; pl->field_bits = 0;
     pl->cluster = 0;
     if (engine == RSOS_ENGINE_RESIDENT) {
@@ -246,6 +251,7 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
     Params &p = c->p;
     p.L = L; p.lgL = ilog2(L); p.N = N; p.R = R; p.first_real = opt.first_real;
     p.S = S; p.lgS = ilog2(S); p.K = K;
+    p.general = pl.general ? 1u : 0u; p.T = pl.T;
     p.k0 = (uint32_t)(seed & 0xFFFFFFFFull); p.k1 = (uint32_t)(seed >> 32);
 
 #define INIT_TRY(expr, code)                                                                             \
@@ -545,7 +551,8 @@ extern "C" int rsos_moments(rsos_ctx *c, int64_t *base, uint64_t *out)
     long long *hb = reinterpret_cast<long long *>(c->h_red + (size_t)p.R * 5);
     for (uint32_t r = 0; r < p.R; ++r) {
         const int64_t s1 = (int64_t)c->h_red[4 * (size_t)r];
-        hb[r] = s1 >> (2 * p.lgL);                                  // floor(S1 / L^2)
+        const int64_t n2 = (int64_t)p.L * p.L;
+        hb[r] = s1 >= 0 ? s1 / n2 : -((-s1 + n2 - 1) / n2);         // floor(S1 / L^2)
         if (base) base[r] = hb[r];
     }
     CUDA_TRY(cudaMemcpyAsync(c->d_base, hb, (size_t)p.R * sizeof(long long), cudaMemcpyHostToDevice, c->stream));

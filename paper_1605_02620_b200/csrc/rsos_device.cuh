@@ -47,6 +47,8 @@ struct Params {
     uint32_t *pk;                   // THREAD engine: packed working lattice, FB bits per site (rsos_pack.cu)
     uint32_t FB;                    // field bits of pk (2 or 4); 0 when there is no packed lattice
     uint32_t KL;                    // THREAD engine: lanes per tile (1, 2, 4 or 8)
+    uint32_t general;               // 1: L is not a power of two -- general-L schedule RSG / DTG (D:2b), SIMPLE engine
+    uint32_t T;                     // general DT mode: tiles per side, 2 * floor(L / 2S)
     uint32_t CS;                    // RESIDENT engine: thread blocks per cluster = per realization (1, 2, 4, 8 or 16)
 };
 
@@ -61,5 +63,36 @@ __device__ __forceinline__ void draw_origin(const Params &p, uint32_t u, uint32_
     ox = o.x & (p.L - 1);
     oy = o.y & (p.L - 1);
 }
+
+// ---------------------------------------------------------------------------------------------
+// General-L schedule (D:2b): lattice sides that are not powers of two (P:79 L = 9605; P:204 irregular
+// tilings).  Word stream of (tile id, u, r): word i = o[i & 3] of Philox(counter (i >> 2, tile id, u, r));
+// draw(n): exactly uniform on [0, n) -- multiply-shift, a word whose low product half is below
+// 2^32 mod n is rejected and the next word of the stream is taken.
+// ---------------------------------------------------------------------------------------------
+struct WordStream {
+    uint32_t q, tile, u, rg, k0, k1, j;
+    uint4 o;
+    __device__ __forceinline__ WordStream(const Params &p, uint32_t tile_id, uint32_t u_, uint32_t rg_)
+        : q(0), tile(tile_id), u(u_), rg(rg_), k0(p.k0), k1(p.k1), j(4), o(make_uint4(0, 0, 0, 0)) {}
+    __device__ __forceinline__ uint32_t next()
+    {
+        if (j == 4) { o = philox4x32_10(q, tile, u, rg, k0, k1); ++q; j = 0; }
+        const uint32_t v = j == 0 ? o.x : j == 1 ? o.y : j == 2 ? o.z : o.w;
+        ++j;
+        return v;
+    }
+    // thr = 2^32 mod n
+    __device__ __forceinline__ uint32_t draw(uint32_t n, uint32_t thr)
+    {
+        for (;;) {
+            const uint64_t m = (uint64_t)next() * n;
+            if ((uint32_t)m >= thr) return (uint32_t)(m >> 32);
+        }
+    }
+};
+
+__device__ __forceinline__ uint32_t pow32_mod(uint32_t n) { return (uint32_t)(0x100000000ull % n); }
+__device__ __forceinline__ uint32_t tile_edge(uint32_t i, uint32_t L, uint32_t T) { return (uint32_t)(((uint64_t)i * L) / T); }
 
 }  // namespace rsos

@@ -10,20 +10,33 @@ namespace rsos {
 
 constexpr int RED_THREADS = 256;
 
-__global__ void __launch_bounds__(RED_THREADS) sums_kernel(const int32_t *__restrict__ h, uint32_t n4 /* L*L/4 */,
+// VEC: n is a multiple of 4 sites per surface (every power-of-two lattice), int4 loads; otherwise (general L with
+// L*L not a multiple of 4, D:2b) one site per load.
+template <bool VEC>
+__global__ void __launch_bounds__(RED_THREADS) sums_kernel(const int32_t *__restrict__ h, uint32_t n /* VEC: L*L/4, else L*L */,
                                                            unsigned long long *out)
 {
     const uint32_t r = blockIdx.y;
-    const int4 *src = reinterpret_cast<const int4 *>(h) + (size_t)r * n4;
     long long s1 = 0;
     unsigned long long s2 = 0;
     unsigned int mx = 0;
-    for (uint32_t i = blockIdx.x * RED_THREADS + threadIdx.x; i < n4; i += gridDim.x * RED_THREADS) {
-        const int4 q = __ldg(src + i);
-        s1 += (long long)q.x + (long long)q.y + (long long)q.z + (long long)q.w;
-        s2 += (unsigned long long)((long long)q.x * q.x) + (unsigned long long)((long long)q.y * q.y) +
-              (unsigned long long)((long long)q.z * q.z) + (unsigned long long)((long long)q.w * q.w);
-        mx = max(max(mx, (unsigned int)abs(q.x)), max((unsigned int)abs(q.y), max((unsigned int)abs(q.z), (unsigned int)abs(q.w))));
+    if (VEC) {
+        const int4 *src = reinterpret_cast<const int4 *>(h) + (size_t)r * n;
+        for (uint32_t i = blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += gridDim.x * RED_THREADS) {
+            const int4 q = __ldg(src + i);
+            s1 += (long long)q.x + (long long)q.y + (long long)q.z + (long long)q.w;
+            s2 += (unsigned long long)((long long)q.x * q.x) + (unsigned long long)((long long)q.y * q.y) +
+                  (unsigned long long)((long long)q.z * q.z) + (unsigned long long)((long long)q.w * q.w);
+            mx = max(max(mx, (unsigned int)abs(q.x)), max((unsigned int)abs(q.y), max((unsigned int)abs(q.z), (unsigned int)abs(q.w))));
+        }
+    } else {
+        const int32_t *src = h + (size_t)r * n;
+        for (uint32_t i = blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += gridDim.x * RED_THREADS) {
+            const int v = __ldg(src + i);
+            s1 += (long long)v;
+            s2 += (unsigned long long)((long long)v * v);
+            mx = max(mx, (unsigned int)abs(v));
+        }
     }
     for (int o = 16; o; o >>= 1) {
         s1 += __shfl_xor_sync(0xFFFFFFFFu, s1, o);
@@ -57,15 +70,17 @@ cudaError_t launch_sums(const int32_t *h, uint32_t L, uint32_t R, unsigned long 
 {
     cudaError_t e = cudaMemsetAsync(d_out, 0, (size_t)R * 4 * sizeof(unsigned long long), st);
     if (e != cudaSuccess) return e;
-    const uint64_t n4 = (uint64_t)L * L / 4;
-    // enough blocks per realization to cover every SM with 8 blocks, at most one block per 256*4 int4
+    const bool vec = ((uint64_t)L * L) % 4 == 0;
+    const uint64_t n4 = vec ? (uint64_t)L * L / 4 : (uint64_t)L * L;
+    // enough blocks per realization to cover every SM with 8 blocks, at most one block per 256*4 loads
     uint64_t bx = (n4 + RED_THREADS * 4 - 1) / (RED_THREADS * 4);
     const uint64_t want = ((uint64_t)(sm_count > 0 ? sm_count : 1) * 8 + R - 1) / R;
     if (bx > want) bx = want;
     if (bx < 1) bx = 1;
     for (uint32_t r0 = 0; r0 < R; r0 += 65535) {
         const uint32_t nr = R - r0 < 65535 ? R - r0 : 65535;
-        sums_kernel<<<dim3((unsigned)bx, nr), RED_THREADS, 0, st>>>(h + (size_t)r0 * L * L, (uint32_t)n4, d_out + 4 * (size_t)r0);
+        if (vec) sums_kernel<true><<<dim3((unsigned)bx, nr), RED_THREADS, 0, st>>>(h + (size_t)r0 * L * L, (uint32_t)n4, d_out + 4 * (size_t)r0);
+        else sums_kernel<false><<<dim3((unsigned)bx, nr), RED_THREADS, 0, st>>>(h + (size_t)r0 * L * L, (uint32_t)n4, d_out + 4 * (size_t)r0);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
@@ -92,22 +107,27 @@ __device__ __forceinline__ __int128 shfl_xor128(__int128 v, int o)
     return (__int128)(((unsigned __int128)hi << 64) | lo);
 }
 
+template <bool VEC>
 __global__ void __launch_bounds__(RED_THREADS) moments_kernel(const int32_t *__restrict__ h, uint32_t n4,
                                                               const long long *__restrict__ base, unsigned long long *out)
 {
     const uint32_t r = blockIdx.y;
-    const int4 *src = reinterpret_cast<const int4 *>(h) + (size_t)r * n4;
     const long long b = base[r];
     __int128 m[4] = {0, 0, 0, 0};
-    for (uint32_t i = blockIdx.x * RED_THREADS + threadIdx.x; i < n4; i += gridDim.x * RED_THREADS) {
-        const int4 q = __ldg(src + i);
-        const int v[4] = {q.x, q.y, q.z, q.w};
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const __int128 d = (long long)v[k] - b;
-            const __int128 d2 = d * d;
-            m[0] += d; m[1] += d2; m[2] += d2 * d; m[3] += d2 * d2;
+    auto add = [&](int v) {
+        const __int128 d = (long long)v - b;
+        const __int128 d2 = d * d;
+        m[0] += d; m[1] += d2; m[2] += d2 * d; m[3] += d2 * d2;
+    };
+    if (VEC) {
+        const int4 *src = reinterpret_cast<const int4 *>(h) + (size_t)r * n4;
+        for (uint32_t i = blockIdx.x * RED_THREADS + threadIdx.x; i < n4; i += gridDim.x * RED_THREADS) {
+            const int4 q = __ldg(src + i);
+            add(q.x); add(q.y); add(q.z); add(q.w);
         }
+    } else {
+        const int32_t *src = h + (size_t)r * n4;
+        for (uint32_t i = blockIdx.x * RED_THREADS + threadIdx.x; i < n4; i += gridDim.x * RED_THREADS) add(__ldg(src + i));
     }
     for (int o = 16; o; o >>= 1)
 #pragma unroll
@@ -122,15 +142,18 @@ cudaError_t launch_moments(const int32_t *h, uint32_t L, uint32_t R, const long 
 {
     cudaError_t e = cudaMemsetAsync(d_out, 0, (size_t)R * 8 * sizeof(unsigned long long), st);
     if (e != cudaSuccess) return e;
-    const uint64_t n4 = (uint64_t)L * L / 4;
+    const bool vec = ((uint64_t)L * L) % 4 == 0;
+    const uint64_t n4 = vec ? (uint64_t)L * L / 4 : (uint64_t)L * L;
     uint64_t bx = (n4 + RED_THREADS * 4 - 1) / (RED_THREADS * 4);
     const uint64_t want = ((uint64_t)(sm_count > 0 ? sm_count : 1) * 8 + R - 1) / R;
     if (bx > want) bx = want;
     if (bx < 1) bx = 1;
     for (uint32_t r0 = 0; r0 < R; r0 += 65535) {
         const uint32_t nr = R - r0 < 65535 ? R - r0 : 65535;
-        moments_kernel<<<dim3((unsigned)bx, nr), RED_THREADS, 0, st>>>(h + (size_t)r0 * L * L, (uint32_t)n4, d_base + r0,
-                                                                       d_out + 8 * (size_t)r0);
+        if (vec) moments_kernel<true><<<dim3((unsigned)bx, nr), RED_THREADS, 0, st>>>(h + (size_t)r0 * L * L, (uint32_t)n4, d_base + r0,
+                                                                                     d_out + 8 * (size_t)r0);
+        else moments_kernel<false><<<dim3((unsigned)bx, nr), RED_THREADS, 0, st>>>(h + (size_t)r0 * L * L, (uint32_t)n4, d_base + r0,
+                                                                                   d_out + 8 * (size_t)r0);
         e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
@@ -144,13 +167,14 @@ cudaError_t launch_moments(const int32_t *h, uint32_t L, uint32_t R, const long 
 __global__ void __launch_bounds__(RED_THREADS) violations_kernel(const int32_t *__restrict__ h, uint32_t L, uint32_t lgL,
                                                                  int32_t N, unsigned long long *d_bad)
 {
-    const int32_t *s = h + ((size_t)blockIdx.y << (2 * lgL));
-    const uint32_t Lm = L - 1;
+    (void)lgL;
+    const uint64_t n = (uint64_t)L * L;
+    const int32_t *s = h + (size_t)blockIdx.y * n;
     unsigned int bad = 0;
-    for (uint64_t i = (uint64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < ((uint64_t)1 << (2 * lgL)); i += (uint64_t)gridDim.x * RED_THREADS) {
-        const uint32_t x = (uint32_t)i & Lm, y = (uint32_t)(i >> lgL);
+    for (uint64_t i = (uint64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (uint64_t)gridDim.x * RED_THREADS) {
+        const uint32_t y = (uint32_t)(i / L), x = (uint32_t)(i - (uint64_t)y * L);      // any L (D:2b)
         const int32_t c = s[i];
-        const int32_t r = s[((size_t)y << lgL) + ((x + 1) & Lm)], d = s[((size_t)((y + 1) & Lm) << lgL) + x];
+        const int32_t r = s[(size_t)y * L + (x + 1 == L ? 0 : x + 1)], d = s[(size_t)(y + 1 == L ? 0 : y + 1) * L + x];
         bad += (abs(c - r) > N) + (abs(c - d) > N);
     }
     for (int o = 16; o; o >>= 1) bad += __shfl_xor_sync(0xFFFFFFFFu, bad, o);

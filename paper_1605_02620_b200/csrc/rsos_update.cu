@@ -54,8 +54,59 @@ __device__ __forceinline__ uint32_t simple_run_tile(const Params &p, int32_t *h,
     return nacc;
 }
 
+// General-L form (D:2b): a tile of w x hgt sites whose first site is (x0, y0); A attempts, each
+// s = draw(w * hgt), dx = s mod w, dy = s div w, site ((x0 + dx) mod L, (y0 + dy) mod L).
+__device__ __forceinline__ uint32_t general_run_tile(const Params &p, int32_t *h, uint32_t rg, uint32_t u, uint32_t tile_id,
+                                                     uint32_t x0, uint32_t y0, uint32_t w, uint32_t hgt, uint64_t A)
+{
+    const uint32_t L = p.L, n = w * hgt, thr = pow32_mod(n);
+    const int32_t N = (int32_t)p.N;
+    WordStream ws(p, tile_id, u, rg);
+    uint32_t nacc = 0;
+    for (uint64_t a = 0; a < A; ++a) {
+        const uint32_t s = ws.draw(n, thr);
+        const uint32_t dy = s / w, dx = s - dy * w;
+        uint32_t x = x0 + dx, y = y0 + dy;
+        if (x >= L) x -= L;
+        if (y >= L) y -= L;
+        const uint32_t xm = x ? x - 1 : L - 1, xp = x + 1 == L ? 0 : x + 1;
+        const uint32_t ym = y ? y - 1 : L - 1, yp = y + 1 == L ? 0 : y + 1;
+        int32_t *row = h + (size_t)y * L;
+        const int32_t c = row[x] + 1;
+        const int32_t l = row[xm], r = row[xp];
+        const int32_t up = h[(size_t)ym * L + x], dn = h[(size_t)yp * L + x];
+        const bool ok = abs(c - l) <= N && abs(c - r) <= N && abs(c - up) <= N && abs(c - dn) <= N;
+        if (ok) { row[x] = c; ++nacc; }
+    }
+    return nacc;
+}
+
+// One colour pass of the general-L DT schedule: T = 2 floor(L / 2S) tiles per side with edges floor(i L / T); the
+// origin of sub-sweep u comes from the stream of tile id 0xFFFFFFFF; in sub-sweep k = u mod K a tile of n sites makes
+// floor((k + 1) n / K) - floor(k n / K) attempts (n per MCS).
+__device__ __forceinline__ void general_dt_pass(const Params &p, uint32_t u, uint32_t colour, uint32_t idx)
+{
+    const uint32_t L = p.L, T = p.T, half = T >> 1, ntile = half * half;
+    if (idx >= p.R * ntile) return;
+    const uint32_t rl = idx / ntile, n = idx - rl * ntile;
+    const uint32_t I = 2 * (n % half) + (colour & 1u), J = 2 * (n / half) + (colour >> 1);
+    const uint32_t rg = p.first_real + rl;
+    WordStream os(p, 0xFFFFFFFFu, u, rg);
+    const uint32_t thrL = pow32_mod(L);
+    const uint32_t ox = os.draw(L, thrL);
+    const uint32_t oy = os.draw(L, thrL);
+    const uint32_t bx = tile_edge(I, L, T), by = tile_edge(J, L, T);
+    const uint32_t w = tile_edge(I + 1, L, T) - bx, hgt = tile_edge(J + 1, L, T) - by;
+    const uint64_t sites = (uint64_t)w * hgt, k = u & (p.K - 1u);
+    const uint64_t A = ((k + 1) * sites) / p.K - (k * sites) / p.K;
+    int32_t *h = p.h + (size_t)rl * L * L;
+    const uint32_t nacc = general_run_tile(p, h, rg, u, J * T + I, (ox + bx) % L, (oy + by) % L, w, hgt, A);
+    if (nacc) atomicAdd(p.accepted + rl, (unsigned long long)nacc);
+}
+
 __global__ void __launch_bounds__(128) simple_dt_kernel(Params p, uint32_t u, uint32_t colour)
 {
+    if (p.general) { general_dt_pass(p, u, colour, blockIdx.x * blockDim.x + threadIdx.x); return; }
     const uint32_t T = p.L >> p.lgS, half = T >> 1, ntile = half * half;
     const uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= p.R * ntile) return;
@@ -78,7 +129,8 @@ __global__ void __launch_bounds__(32) simple_rs_kernel(Params p, uint32_t t0, ui
     int32_t *h = p.h + (size_t)rl * p.L * p.L;
     unsigned long long nacc = 0;
     for (uint32_t m = 0; m < mcs; ++m)
-        nacc += simple_run_tile(p, h, p.first_real + rl, t0 + m, 0u, 0u, 0u, p.L, p.lgL, (uint64_t)p.L * p.L);
+        nacc += p.general ? general_run_tile(p, h, p.first_real + rl, t0 + m, 0u, 0u, 0u, p.L, p.L, (uint64_t)p.L * p.L)
+                          : simple_run_tile(p, h, p.first_real + rl, t0 + m, 0u, 0u, 0u, p.L, p.lgL, (uint64_t)p.L * p.L);
     if (nacc) atomicAdd(p.accepted + rl, nacc);
 }
 
@@ -500,7 +552,7 @@ cudaError_t configure_engine(const Params &p, uint32_t engine, bool mode_dt)
 
 uint32_t engine_blocks(const Params &p, uint32_t engine, bool mode_dt)
 {
-    const uint32_t T = p.L >> p.lgS, half = T >> 1;
+    const uint32_t T = p.general ? p.T : p.L >> p.lgS, half = T >> 1;
     const uint64_t tiles = mode_dt ? (uint64_t)p.R * half * half : p.R;
     if (engine == ENGINE_THREAD) return thread_dt_blocks(p);
     if (engine == ENGINE_RESIDENT) return resident_blocks(p);

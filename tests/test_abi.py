@@ -61,7 +61,8 @@ def test_no_cpu_fallback_without_a_device():
 
 def test_argument_errors_need_no_device(lib_path):
     import paper_1605_02620_b200 as m
-    for args, kw, code in [((48, 1, 1, 1), {}, -1), ((64, 0, 1, 1), {}, -1), ((64, 1, 0, 1), {}, -1),
+    for args, kw, code in [((3, 1, 1, 1), {}, -1), ((70000, 1, 1, 1), {}, -1), ((48, 1, 1, 1), dict(engine=m.ENGINE_ONCHIP), -5),
+                           ((150, 1, 1, 1), dict(engine=m.ENGINE_THREAD), -5), ((64, 0, 1, 1), {}, -1), ((64, 1, 0, 1), {}, -1),
                            ((128, 1, 1, 1), dict(tile=24), -1), ((64, 1, 1, 1), dict(engine=m.ENGINE_WARP), -5),
                            ((256, 1, 1, 1), dict(engine=m.ENGINE_ONCHIP), -5), ((128, 32, 1, 1), dict(engine=m.ENGINE_WARP), -5),
                            ((128, 1, 1, 1), dict(lanes=3), -1), ((128, 8, 1, 1), dict(engine=m.ENGINE_THREAD), -5),
@@ -119,5 +120,10 @@ def test_plan_picks_engines_lanes_and_site_width(lib_path):
     with pytest.raises(m.RsosError) as e:
         m.plan(1024, 1, 128, subsweeps=128, engine=m.ENGINE_THREAD, lanes=8)         # a batch of 64 attempts does not fit
     assert e.value.code == -1
+    # lattice sides that are not powers of two: the general-L schedule, SIMPLE engine
+    p = m.plan(9605, 1, 128)
+    assert (p["mode"], p["engine"], p["S"], p["pass_tiles"]) == ("DT", "simple", 64, 128 * 75 * 75)
+    p = m.plan(100, 1, 4)
+    assert (p["mode"], p["engine"], p["S"]) == ("RS", "simple", 100)
     # fewer SMs: the same pass reaches six warps per SM with fewer lanes
     assert m.plan(c["C2"]["L"], 1, c["C2"]["R"], sm_count=16)["lanes"] == 2

@@ -1,0 +1,98 @@
+"""GPU parity for lattice sides that are not powers of two (S 8(f) NEXT-3): the general-L
+schedule RSG / DTG through the C ABI against the CPU oracle, bit-exact (heights, S1, S2, accepted, W2 / <h>
+doubles, power sums), including the paper's largest system L = 9605 for a prefix."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def rsos():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1605_02620_b200 import build
+    build.build()
+    import paper_1605_02620_b200 as m
+    return m
+
+
+def _same(g, o, R):
+    for a, b in zip(g.sums(), o.sums()):
+        assert (a == b).all()
+    gw, gh = g.width()
+    ow, oh = o.width()
+    assert (gw == ow).all() and (gh == oh).all()
+    assert np.array_equal(g.heights(), o.heights())
+
+
+@pytest.mark.parametrize("L,N,R,S,K,mcs,first", [
+    (150, 1, 3, 64, 1, 5, 0),        # DTG, T = 2, four tiles of 75 x 75
+    (200, 2, 2, 32, 4, 4, 5),        # DTG, T = 6, widths 33 / 34, four sub-sweeps of unequal attempt counts
+    (100, 1, 2, 8, 2, 3, 0),         # DTG, T = 12
+    (333, 3, 1, 16, 1, 2, 1),        # DTG, T = 20, odd L: scalar reductions
+    (45, 1, 4, 64, 1, 12, 0),        # RSG (2S > L), odd L
+    (6, 1, 5, 64, 1, 40, 2),         # RSG, tiny
+])
+def test_general_lattice_equals_oracle(rsos, oracle_mod, L, N, R, S, K, mcs, first):
+    g = rsos.Rsos(L, N, R, 3, tile=S, subsweeps=K, first_real=first)
+    o = oracle_mod.Oracle(L, N, R, 3, tile=S, subsweeps=K, first_real=first)
+    info = g.info()
+    assert info["engine"] == "simple" and info["mode"] == o.mode
+    for step in (1, mcs - 1):
+        g.advance(step)
+        o.advance(step)
+        _same(g, o, R)
+    base, M = g.moments()
+    for r in range(R):
+        assert M[r] == o.power_sums(r, int(base[r]))
+    g.close()
+    o.close()
+
+
+def test_general_lattice_snapshot_restart(rsos, oracle_mod):
+    """set_state / get_heights on a general lattice: the oracle continues from a GPU snapshot (t enters the counter)."""
+    L, N, R = 150, 1, 2
+    g = rsos.Rsos(L, N, R, 8)
+    g.advance(7)
+    snap, (_, _, acc) = g.heights(), g.sums()
+    o = oracle_mod.Oracle(L, N, R, 8)
+    o.set_state(snap, 7, acc)
+    g.advance(3)
+    o.advance(3)
+    _same(g, o, R)
+    g2 = rsos.Rsos(L, N, R, 8)
+    g2.set_state(snap, 7, acc)
+    g2.advance(3)
+    _same(g2, o, R)
+    bad = snap.copy()
+    bad[0, 0, 0] += 5
+    with pytest.raises(rsos.RsosError) as e:
+        g2.set_state(bad, 7, acc)
+    assert e.value.code == rsos.binding.RSOS_EINVAL
+    for x in (g, g2):
+        x.close()
+    o.close()
+
+
+def test_general_lattice_refuses_other_engines(rsos):
+    for eng in (rsos.ENGINE_THREAD, rsos.ENGINE_WARP, rsos.ENGINE_RESIDENT, rsos.ENGINE_ONCHIP):
+        with pytest.raises(rsos.RsosError) as e:
+            rsos.Rsos(150, 1, 1, 1, engine=eng)
+        assert e.value.code == rsos.binding.RSOS_EUNSUP
+
+
+def test_paper_largest_system_prefix(rsos, oracle_mod):
+    """L = 9605 ('bounded by memory constraints'), N = 1, one realization, DTG(64,1): 150 x 150 tiles of 64 / 65
+    sites, 5625 per colour pass; 2 MCS = 1.8e8 attempts, every height compared with the oracle."""
+    L = 9605
+    g = rsos.Rsos(L, 1, 1, 1)
+    o = oracle_mod.Oracle(L, 1, 1, 1)
+    g.advance(2)
+    o.advance(2)
+    _same(g, o, 1)
+    W2, hm = g.width()
+    assert 0.3 < W2[0] < 0.4 and 1.0 < hm[0] < 1.2           # W^2(2) = 0.339 on a large lattice (C2 time series)
+    g.close()
+    o.close()
