@@ -49,7 +49,8 @@ enum {
 /* Update engines.  All of them produce bit-identical heights (tests/test_gpu_parity.py).       */
 enum {
     RSOS_ENGINE_AUTO   = 0,  /* RS mode: ONCHIP when the lattice fits in shared memory, else      */
-                             /* SIMPLE.  DT mode: THREAD when it applies and one colour pass has  */
+                             /* SIMPLE.  DT mode: FINE when it applies (tile 8 or 16, L <= 512),  */
+                             /* else THREAD when it applies and one colour pass has               */
                              /* at least RSOS_THREAD_MIN_TILES active tiles, else RESIDENT when   */
                              /* it applies, else WARP, else SIMPLE                                */
     RSOS_ENGINE_SIMPLE = 1,  /* one thread per active tile, heights in global memory (slow;       */
@@ -63,6 +64,10 @@ enum {
     RSOS_ENGINE_THREAD = 4,  /* DT mode: one thread per active tile, the tile window held in      */
                              /* bank-interleaved shared memory at 2 (N = 1) or 4 (N <= 7) bits    */
                              /* per site; needs tile <= 64 and N <= 7                             */
+    RSOS_ENGINE_FINE = 6,    /* DT mode with the paper's small sequential units ("domain sizes of 8 x 8  */
+                             /* lattice sites", P:204 16 x 16): tile = 8 or 16, N <= 7, L <= 512.  One thread */
+                             /* per cell works straight on a 4-bit lattice that stays in shared memory for    */
+                             /* all passes of an rsos_advance call (one or more realizations per block)       */
     RSOS_ENGINE_RESIDENT = 5 /* DT mode, small lattices: a cluster of thread blocks keeps the     */
                              /* lattice of one realization in (distributed) shared memory for     */
                              /* every colour pass, sub-sweep and MCS of an rsos_advance call; one */

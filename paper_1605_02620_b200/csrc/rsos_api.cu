@@ -121,7 +121,7 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
         return fail(RSOS_EINVAL, "opts.lanes = %u must be 0, 1, 2, 4 or 8", opt.lanes);
     if (opt.cluster != 0 && opt.cluster != 1 && opt.cluster != 2 && opt.cluster != 4 && opt.cluster != 8 && opt.cluster != 16)
         return fail(RSOS_EINVAL, "opts.cluster = %u must be 0, 1, 2, 4, 8 or 16", opt.cluster);
-    if (opt.engine > RSOS_ENGINE_RESIDENT) return fail(RSOS_EINVAL, "unknown engine %u", opt.engine);
+    if (opt.engine > RSOS_ENGINE_FINE) return fail(RSOS_EINVAL, "unknown engine %u", opt.engine);
     uint32_t S = opt.tile ? opt.tile : 64, K = opt.subsweeps ? opt.subsweeps : 1;
     if (!is_pow2(S) || S < 8) return fail(RSOS_EINVAL, "tile = %u must be a power of two >= 8", S);
     if (!is_pow2(K)) return fail(RSOS_EINVAL, "subsweeps = %u must be a power of two", K);
@@ -149,8 +149,10 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
         if (opt.cluster) { if (resident_ok(L, N, S, K, opt.cluster, smem_limit)) res_cluster = opt.cluster; }
         else res_cluster = resident_cluster_size(L, N, S, K, R, sm_count, smem_limit);
     }
+    const bool fine_can = !general && mode_dt && fine_ok(L, N, S, K);
     if (engine == RSOS_ENGINE_AUTO) {
         if (!mode_dt) engine = onchip_ok ? RSOS_ENGINE_ONCHIP : RSOS_ENGINE_SIMPLE;
+        else if (fine_can) engine = RSOS_ENGINE_FINE;                  // 8- or 16-site cells on a lattice that fits on chip
         else if (thread_ok && pass_tiles >= RSOS_THREAD_MIN_TILES) engine = RSOS_ENGINE_THREAD;
         else if (res_cluster && pass_tiles / R <= 16) engine = RSOS_ENGINE_RESIDENT;   // few tiles per pass and realization
         else engine = warp_ok ? RSOS_ENGINE_WARP : thread_ok ? RSOS_ENGINE_THREAD : RSOS_ENGINE_SIMPLE;
@@ -158,6 +160,8 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
     if (engine == RSOS_ENGINE_RESIDENT && !res_cluster)
         return fail(RSOS_EUNSUP, "engine RESIDENT needs DT mode, 16 <= tile <= 64, N <= 7, a cluster size of 1, 2, 4, 8 or 16 that divides "
                                  "the (L / 2 tile)^2 tiles of a colour pass with at most 16 tiles per block, and the lattice slab in shared memory");
+    if (engine == RSOS_ENGINE_FINE && !fine_can)
+        return fail(RSOS_EUNSUP, "engine FINE needs DT mode with tile 8 or 16, N <= 7 and L <= 512 (the 4-bit lattice within 128 KiB)");
     if (engine == RSOS_ENGINE_WARP && !warp_ok)
         return fail(RSOS_EUNSUP, "engine WARP needs DT mode (2*tile <= L), tile <= 128 and N <= 31");
     if (engine == RSOS_ENGINE_THREAD && !thread_ok)
@@ -174,6 +178,10 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
         pl->field_bits = thread_dt_field_bits(N, S);
         pl->lanes = 32;                                    // one warp per tile
         pl->cluster = res_cluster;
+    }
+    if (engine == RSOS_ENGINE_FINE) {
+        pl->field_bits = thread_dt_field_bits(N, S);
+        pl->lanes = 1;                                     // one thread per cell
     }
     if (engine == RSOS_ENGINE_THREAD) {
         pl->field_bits = thread_dt_field_bits(N, S);
@@ -207,7 +215,7 @@ extern "C" int rsos_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts *o,
     if (rc) return rc;
     out[0] = pl.mode_dt ? 1 : 0; out[1] = pl.engine; out[2] = pl.S; out[3] = pl.K;
     out[4] = pl.pass_tiles; out[5] = pl.lanes; out[6] = pl.field_bits;
-    out[7] = pl.engine == RSOS_ENGINE_RESIDENT ? 1 : pl.mode_dt ? (uint64_t)4 * pl.K : 1;      // launches per MCS (RESIDENT, RS: per call)
+    out[7] = (pl.engine == RSOS_ENGINE_RESIDENT || pl.engine == RSOS_ENGINE_FINE) ? 1 : pl.mode_dt ? (uint64_t)4 * pl.K : 1;      // launches per MCS (RESIDENT, RS: per call)
     out[8] = pl.cluster;
     return RSOS_OK;
 }
@@ -267,7 +275,7 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
     } while (0)
 
     const size_t bytes = (size_t)R * L * L * sizeof(int32_t);
-    const bool packed_state = engine == RSOS_ENGINE_THREAD || engine == RSOS_ENGINE_RESIDENT;   // working state = packed lattice (D:5)
+    const bool packed_state = engine == RSOS_ENGINE_THREAD || engine == RSOS_ENGINE_RESIDENT || engine == RSOS_ENGINE_FINE;   // working state = packed lattice (D:5)
     if (opt.d_heights) { p.h = opt.d_heights; c->own_heights = false; }
     else if (!packed_state) { INIT_TRY(cudaMalloc(&p.h, bytes), RSOS_ECUDA); c->own_heights = true; }
     // else: the int32 heights are allocated by the first call that needs them (alloc_heights)
@@ -296,12 +304,14 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
     INIT_TRY(cudaMemsetAsync(p.accepted, 0, (size_t)R * sizeof(unsigned long long), c->stream), RSOS_ECUDA);
     INIT_TRY(cudaMemsetAsync(p.err, 0, sizeof(uint32_t), c->stream), RSOS_ECUDA);
     INIT_TRY(cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev), RSOS_ECUDA);
+    p.sm_count = (uint32_t)c->sm_count;
     INIT_TRY(configure_engine(p, engine, mode_dt), RSOS_ECUDA);
     c->blocks = engine_blocks(p, engine, mode_dt);
     INIT_TRY(cudaEventCreate(&c->ev0), RSOS_ECUDA);
     INIT_TRY(cudaEventCreate(&c->ev1), RSOS_ECUDA);
     c->smem_bytes = engine == RSOS_ENGINE_WARP ? warp_dt_smem(p.lgS) : engine == RSOS_ENGINE_ONCHIP ? warp_rs_smem(p.lgL)
-                    : engine == RSOS_ENGINE_THREAD ? thread_dt_smem(p) : engine == RSOS_ENGINE_RESIDENT ? resident_smem(p) : 0;
+                    : engine == RSOS_ENGINE_THREAD ? thread_dt_smem(p) : engine == RSOS_ENGINE_RESIDENT ? resident_smem(p)
+                    : engine == RSOS_ENGINE_FINE ? fine_smem(p) : 0;
 #undef INIT_TRY
     *out = c;
     return RSOS_OK;
@@ -403,14 +413,15 @@ extern "C" int rsos_advance(rsos_ctx *c, uint64_t mcs)
         CUDA_TRY(cudaEventRecord(c->ev0, c->stream));
         c->launches_at_ev0 = c->launches;
     }
-    if (c->engine == RSOS_ENGINE_RESIDENT) {
+    if (c->engine == RSOS_ENGINE_RESIDENT || c->engine == RSOS_ENGINE_FINE) {
         // all colour passes and sub-sweeps of many MCS inside one launch; long calls are cut into launches of
         // about 2^36 attempts (a fraction of a second) so that the stream stays responsive
         const uint64_t per_mcs = (uint64_t)p.R * p.L * p.L;
         const uint64_t chunk = per_mcs >= (1ull << 36) ? 1 : (1ull << 36) / per_mcs;
         for (uint64_t m = 0; m < mcs; m += chunk) {
             const uint64_t n = mcs - m < chunk ? mcs - m : chunk;
-            CUDA_TRY(resident_launch(p, (uint32_t)(c->t + m), (uint32_t)n, c->stream));
+            if (c->engine == RSOS_ENGINE_FINE) CUDA_TRY(fine_launch(p, (uint32_t)(c->t + m), (uint32_t)n, c->stream));
+            else CUDA_TRY(resident_launch(p, (uint32_t)(c->t + m), (uint32_t)n, c->stream));
             ++c->launches;
         }
     } else if (c->mode_dt) {

@@ -557,3 +557,48 @@ def test_largest_lattice_properties(rsos):
     w2, hm = g.width()
     assert abs(w2[0] / 0.265867 - 1) < 4e-4 and abs(hm[0] / (0.65226 * (1 - 0.00101)) - 1) < 4e-4, (w2, hm)
     g.close()
+
+
+@pytest.mark.parametrize("L,N,R,S,K,mcs,seed", [
+    (64, 1, 5, 8, 1, 6, 1),          # the paper's 8 x 8 domains: 16 cells per pass, several realizations per block
+    (128, 1, 70, 8, 2, 4, 2),        # 16 realizations per block, ragged last block (70 = 4 * 16 + 6)
+    (256, 3, 3, 16, 4, 4, 3),        # 16 x 16 cells, 4-bit sites, K = 4
+    (512, 1, 2, 16, 1, 3, 4),        # 128 KiB lattice per block, 2-bit packed lattice spread to nibbles
+    (512, 2, 1, 8, 1, 2, 5),         # 1024 cells per pass: one thread each
+    (32, 1, 100, 8, 1, 8, 6),        # 4 cells per pass, 100 realizations in one block (400 threads)
+    (16, 7, 9, 8, 2, 10, 7),         # one cell per pass; largest N
+    (64, 1, 3, 16, 8, 5, 8),         # 32 attempts per cell and pass
+])
+def test_dt_fine_engine_equals_oracle(rsos, oracle_mod, L, N, R, S, K, mcs, seed):
+    """The FINE engine (rsos_fine.cu): DT(c, K) with c = 8 or 16, one thread per cell on a 4-bit lattice resident in
+    shared memory for all passes of a call; engine = auto picks it for these shapes."""
+    g = rsos.Rsos(L, N, R, seed, tile=S, subsweeps=K, first_real=seed)
+    o = oracle_mod.Oracle(L, N, R, seed, tile=S, subsweeps=K, first_real=seed)
+    info = g.info()
+    assert info["mode"] == "DT" and info["engine"] == "fine" and not info["int32_allocated"], info
+    for step in (1, 1, mcs - 2):
+        g.advance(step)
+        o.advance(step)
+        compare(g, o, "DT fine L=%d N=%d S=%d K=%d t=%d" % (L, N, S, K, g.t))
+    g.close()
+
+
+def test_dt_fine_engine_saturated_restart_and_cross_engine(rsos, oracle_mod):
+    """FINE engine far from the flat start (L = 64, N = 1, DT(8,1), t = 3000: |h| ~ 900, saturated): snapshot to the
+    oracle, both advance; and the THREAD engine run on the same schedule gives the same surface."""
+    L, N, R, seed = 64, 1, 6, 13
+    g = rsos.Rsos(L, N, R, seed, tile=8)
+    assert g.info()["engine"] == "fine"
+    g.advance(3000)
+    h, (_, _, acc) = g.heights(), g.sums()
+    assert h.min() > 500
+    o = oracle_mod.Oracle(L, N, R, seed, tile=8)
+    o.set_state(h, 3000, acc)
+    t = rsos.Rsos(L, N, R, seed, tile=8, engine=rsos.ENGINE_THREAD)
+    t.set_state(h, 3000, acc)
+    for x in (g, o, t):
+        x.advance(3)
+    compare(g, o, "fine saturated")
+    compare(t, o, "thread on the same cells")
+    g.close()
+    t.close()
