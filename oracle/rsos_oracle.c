@@ -114,6 +114,7 @@ typedef struct rsos_oracle {
     int      mode_dt;        /* 1 = DT(S,K) (DTG when L is not a power of two), 0 = RS (2S > L) */
     int      pow2;           /* L is a power of two                                          */
     uint32_t T;              /* general-L DT mode: tiles per side (even); 0 otherwise        */
+    int      poisson;        /* 1 = DTP(c): Poisson(4) attempts per cell and sub-sweep (D:2c) */
     uint32_t lgL, lgS;
     int32_t *h;              /* R * L * L                                                    */
     int64_t *accepted;       /* R                                                            */
@@ -362,6 +363,39 @@ static void one_mcs_general(rsos_oracle *c, uint32_t rl, uint64_t t, int par_til
     }
 }
 
+/* ------------------------------------------------------------------------------------------
+ * Poisson variant DTP(c) of the DT schedule ("16 passes per MCS,
+ * new origin per pass, Poisson(4) attempts per cell per pass ... matches serial"): K = c*c/4 sub-sweeps
+ * per MCS, each with its own origin, and in every sub-sweep a cell makes n attempts with n drawn from
+ * the Poisson distribution of mean 4 instead of exactly c*c/K = 4.  The count comes from the first
+ * word w of Philox(counter (0xFFFFFFFF, tile id, u, r)) by inversion with the 32-bit table
+ *     POISSON4[k] = floor(2^32 * P(X <= k)),  X ~ Poisson(4),  k = 0 .. 22:   n = #{k : w >= POISSON4[k]}
+ * (so P(n <= k) = POISSON4[k] / 2^32; the table is pinned against a 60-digit evaluation in
+ * tests/test_oracle_poisson.py).  The n attempts then take the slots 0 .. n-1 of the cell exactly as in DT
+ * (slot a mod 8 of call a div 8).  Thinning: every site of the cell gets Poisson(4 / c^2) attempts per
+ * sub-sweep, independently of the others -- Poisson(1) per MCS, which is what serial random-sequential
+ * deposition gives in the large-lattice limit; the fixed count of DT gives Binomial(c^2, 1/c^2).
+ * ------------------------------------------------------------------------------------------ */
+static const uint32_t POISSON4[23] = {
+    78665070u, 393325350u, 1022645910u, 1861739990u, 2700834071u, 3372109335u, 3819626178u, 4075350088u,
+    4203212043u, 4260039579u, 4282770593u, 4291036416u, 4293791691u, 4294639467u, 4294881689u, 4294946282u,
+    4294962430u, 4294966230u, 4294967074u, 4294967252u, 4294967287u, 4294967294u, 4294967295u };
+
+uint32_t rsos_oracle_poisson4(uint32_t w)
+{
+    uint32_t n = 0;
+    for (int k = 0; k < 23; ++k) n += (w >= POISSON4[k]);
+    return n;
+}
+
+int rsos_oracle_set_poisson(rsos_oracle *c, int on)
+{
+    if (on && (!c->mode_dt || !c->pow2)) { snprintf(g_err, sizeof g_err, "DTP needs DT mode on a power-of-two lattice"); return -1; }
+    c->poisson = on ? 1 : 0;
+    if (on) c->K = c->S * c->S / 4;                 /* mean 4 attempts per cell and sub-sweep */
+    return 0;
+}
+
 static uint64_t splitmix64(uint64_t *s)
 { uint64_t z = (*s += 0x9E3779B97F4A7C15ull); z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
   z = (z ^ (z >> 27)) * 0x94D049BB133111EBull; return z ^ (z >> 31); }
@@ -384,7 +418,7 @@ static void one_mcs(rsos_oracle *c, uint32_t rl, uint64_t t, int par_tiles)
         return;
     }
     const uint32_t T = L / S, half = T / 2, ntile = half * half;
-    const uint64_t A = (uint64_t)S * S / K;
+    const uint64_t A_fixed = (uint64_t)S * S / K;
     const uint32_t key[2] = { (uint32_t)(c->seed & 0xffffffffu), (uint32_t)(c->seed >> 32) };
     uint32_t *order = (uint32_t *)malloc(sizeof(uint32_t) * ntile);
     for (uint32_t k = 0; k < K; ++k) {
@@ -409,6 +443,12 @@ static void one_mcs(rsos_oracle *c, uint32_t rl, uint64_t t, int par_tiles)
                 uint32_t i = order[n] % half, j = order[n] / half;
                 uint32_t I = 2 * i + (p & 1), J = 2 * j + (p >> 1);
                 uint32_t x0 = (ox + I * S) & (L - 1), y0 = (oy + J * S) & (L - 1);
+                uint64_t A = A_fixed;
+                if (c->poisson) {                   /* D:2c: the cell's attempt count of this sub-sweep */
+                    uint32_t cctr[4] = { 0xFFFFFFFFu, J * T + I, u, rg }, co[4];
+                    rsos_oracle_philox(cctr, key, co);
+                    A = rsos_oracle_poisson4(co[0]);
+                }
                 acc += run_tile(c, h, rg, u, J * T + I, x0, y0, S, c->lgS, A);
             }
             c->accepted[rl] += acc;

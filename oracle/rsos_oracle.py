@@ -69,12 +69,21 @@ def lib():
         l.rsos_oracle_height_moments.restype = C.c_int
         l.rsos_oracle_power_sums.argtypes = [vp, u32, i64, C.POINTER(u64)]
         l.rsos_oracle_power_sums.restype = C.c_int
+        l.rsos_oracle_poisson4.argtypes = [u32]
+        l.rsos_oracle_poisson4.restype = u32
+        l.rsos_oracle_set_poisson.argtypes = [vp, C.c_int]
+        l.rsos_oracle_set_poisson.restype = C.c_int
         l.rsos_oracle_bounded.argtypes = [u32, u32, C.POINTER(C.c_int)]
         l.rsos_oracle_bounded.restype = u32
         l.rsos_oracle_bounded_census.argtypes = [u32, vp, C.POINTER(u64)]
         l.rsos_oracle_bounded_census.restype = None
         _lib = l
     return _lib
+
+
+def poisson4(w):
+    """Attempt count of the Poisson variant DTP for the 32-bit word w."""
+    return int(lib().rsos_oracle_poisson4(int(w) & 0xFFFFFFFF))
 
 
 def bounded(v, n):
@@ -116,7 +125,7 @@ class Oracle:
     """Same five logical operations as the C-ABI library (init / advance / width / sums / state)."""
 
     def __init__(self, L, N, R, seed, tile=64, subsweeps=1, first_real=0, threads=0,
-                 check_each=False, shuffle_seed=0):
+                 check_each=False, shuffle_seed=0, poisson=False):
         self.L, self.N, self.R, self.seed = int(L), int(N), int(R), int(seed)
         self._l = lib()
         self._c = self._l.rsos_oracle_create(self.L, self.N, self.R, self.seed, int(tile), int(subsweeps),
@@ -124,6 +133,8 @@ class Oracle:
         if not self._c:
             raise ValueError("rsos_oracle_create: " + self._l.rsos_oracle_last_error().decode())
         self._l.rsos_oracle_set_debug(self._c, int(bool(check_each)), int(shuffle_seed), int(threads))
+        if poisson and self._l.rsos_oracle_set_poisson(self._c, 1) != 0:
+            raise ValueError("rsos_oracle_set_poisson: " + self._l.rsos_oracle_last_error().decode())
 
     def close(self):
         if self._c:
