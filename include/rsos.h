@@ -95,6 +95,11 @@ typedef struct rsos_opts {
     uint32_t lanes;       /* THREAD engine: lanes that share one tile, 1, 2, 4 or 8 (8 * lanes must not   */
                           /* exceed tile^2 / subsweeps); 0 = chosen from the number of tiles per colour   */
                           /* pass (D:4).  Does not change the result.                                     */
+    uint32_t poisson;     /* 1: the Poisson variant DTP(c) of the schedule (D:2c): tile = 8 or 16,  */
+                          /* K = tile^2 / 4 sub-sweeps per MCS (subsweeps must be 0 or that value), and in every   */
+                          /* sub-sweep a cell makes n ~ Poisson(4) attempts instead of exactly 4.  Agrees with     */
+                          /* serial dynamics where fixed counts on such small cells are 3.6 % low in W^2; the      */
+                          /* number of attempts per MCS is L^2 on average only.  FINE engine (L <= 512, N <= 7).   */
     uint32_t cluster;     /* RESIDENT engine: thread blocks per realization (a thread-block cluster that  */
                           /* shares its shared memory), 1, 2, 4, 8 or 16; must divide the (L / 2 tile)^2  */
                           /* tiles of a colour pass; 0 = chosen by the library.  Does not change the      */

@@ -124,12 +124,19 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
     if (opt.engine > RSOS_ENGINE_FINE) return fail(RSOS_EINVAL, "unknown engine %u", opt.engine);
     uint32_t S = opt.tile ? opt.tile : 64, K = opt.subsweeps ? opt.subsweeps : 1;
     if (!is_pow2(S) || S < 8) return fail(RSOS_EINVAL, "tile = %u must be a power of two >= 8", S);
+    if (opt.poisson > 1) return fail(RSOS_EINVAL, "opts.poisson = %u must be 0 or 1", opt.poisson);
+    if (opt.poisson) {                                     // D:2c: K = tile^2 / 4 sub-sweeps of Poisson(4) attempts per cell
+        if (S != 8 && S != 16) return fail(RSOS_EINVAL, "opts.poisson needs tile = 8 or 16");
+        if (opt.subsweeps && opt.subsweeps != S * S / 4) return fail(RSOS_EINVAL, "opts.poisson fixes subsweeps = tile^2 / 4 = %u", S * S / 4);
+        K = S * S / 4;
+    }
     if (!is_pow2(K)) return fail(RSOS_EINVAL, "subsweeps = %u must be a power of two", K);
     const bool mode_dt = 2ull * S <= L;
     if (mode_dt) {
-        if (((uint64_t)S * S) % K || (uint64_t)S * S / K < 32)
+        if (!opt.poisson && (((uint64_t)S * S) % K || (uint64_t)S * S / K < 32))
             return fail(RSOS_EINVAL, "subsweeps = %u must divide tile^2 with tile^2/subsweeps >= 32", K);
     } else {
+        if (opt.poisson) return fail(RSOS_EINVAL, "opts.poisson needs DT mode (2 * tile <= L)");
         S = L; K = 1;
     }
     if ((uintptr_t)opt.d_heights & 15u) return fail(RSOS_EINVAL, "d_heights must be 16-byte aligned");
@@ -149,7 +156,11 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
         if (opt.cluster) { if (resident_ok(L, N, S, K, opt.cluster, smem_limit)) res_cluster = opt.cluster; }
         else res_cluster = resident_cluster_size(L, N, S, K, R, sm_count, smem_limit);
     }
-    const bool fine_can = !general && mode_dt && fine_ok(L, N, S, K);
+    const bool fine_can = !general && mode_dt && fine_ok(L, N, S, K, opt.poisson != 0);
+    if (opt.poisson && !fine_can)
+        return fail(RSOS_EUNSUP, "opts.poisson runs on the FINE engine: L <= 512 (a power of two) and N <= 7");
+    if (opt.poisson && engine != RSOS_ENGINE_AUTO && engine != RSOS_ENGINE_FINE)
+        return fail(RSOS_EUNSUP, "opts.poisson runs on the FINE engine only");
     if (engine == RSOS_ENGINE_AUTO) {
         if (!mode_dt) engine = onchip_ok ? RSOS_ENGINE_ONCHIP : RSOS_ENGINE_SIMPLE;
         else if (fine_can) engine = RSOS_ENGINE_FINE;                  // 8- or 16-site cells on a lattice that fits on chip
@@ -260,6 +271,7 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
     p.L = L; p.lgL = ilog2(L); p.N = N; p.R = R; p.first_real = opt.first_real;
     p.S = S; p.lgS = ilog2(S); p.K = K;
     p.general = pl.general ? 1u : 0u; p.T = pl.T;
+    p.poisson = opt.poisson ? 1u : 0u;
     p.k0 = (uint32_t)(seed & 0xFFFFFFFFull); p.k1 = (uint32_t)(seed >> 32);
 
 #define INIT_TRY(expr, code)                                                                             \

@@ -54,7 +54,22 @@ __device__ __forceinline__ uint32_t gather8(uint32_t x)
     return (x | (x >> 8)) & 0xFFFFu;
 }
 
-template <int LGC, int FB>
+// Poisson variant DTP(c) (D:2c): attempt count of a cell in one sub-sweep from the 32-bit word w by inversion,
+// n = #{k : w >= floor(2^32 P(X <= k))}, X ~ Poisson(4), k = 0 .. 22.
+__constant__ uint32_t FINE_POISSON4[23] = {
+    78665070u, 393325350u, 1022645910u, 1861739990u, 2700834071u, 3372109335u, 3819626178u, 4075350088u,
+    4203212043u, 4260039579u, 4282770593u, 4291036416u, 4293791691u, 4294639467u, 4294881689u, 4294946282u,
+    4294962430u, 4294966230u, 4294967074u, 4294967252u, 4294967287u, 4294967294u, 4294967295u};
+
+__device__ __forceinline__ uint32_t poisson4_count(uint32_t w)
+{
+    uint32_t n = 0;
+#pragma unroll
+    for (int k = 0; k < 23; ++k) n += w >= FINE_POISSON4[k] ? 1u : 0u;
+    return n;
+}
+
+template <int LGC, int FB, bool POISSON>
 __global__ void __launch_bounds__(1024) fine_dt_kernel(Params p, uint32_t t0, uint32_t mcs, FineShape sh)
 {
     constexpr uint32_t C = 1u << LGC, M = (1u << FB) - 1u;
@@ -96,28 +111,43 @@ __global__ void __launch_bounds__(1024) fine_dt_kernel(Params p, uint32_t t0, ui
                 const uint32_t I = 2u * a_ + (colour & 1u), J = 2u * b_ + (colour >> 1);
                 const uint32_t x0 = (ox + I * C) & Lm, y0 = (oy + J * C) & Lm;
                 const uint32_t tile_id = J * T + I;
+                // one attempt with the 16-bit slot v (D:2 step 6); returns 1 if accepted
+                auto attempt = [&](uint32_t v) -> uint32_t {
+                    const uint32_t x = (x0 + (v & (C - 1u))) & Lm, y = (y0 + ((v >> LGC) & (C - 1u))) & Lm;
+                    const uint32_t rowb = latb + (y << (lgL - 1u));
+                    const uint32_t aC = rowb + (x >> 1);
+                    const uint32_t bC = fine_lds_u8(aC);
+                    const uint32_t bL = fine_lds_u8(rowb + (((x - 1u) & Lm) >> 1));
+                    const uint32_t bR = fine_lds_u8(rowb + (((x + 1u) & Lm) >> 1));
+                    const uint32_t bU = fine_lds_u8(latb + (((y - 1u) & Lm) << (lgL - 1u)) + (x >> 1));
+                    const uint32_t bD = fine_lds_u8(latb + (((y + 1u) & Lm) << (lgL - 1u)) + (x >> 1));
+                    const uint32_t s = (x & 1u) * 4u, sn = 4u - s;       // my nibble; x - 1 and x + 1 sit in the other one
+                    const uint32_t c = bC >> s;
+                    const uint32_t tq = (c - N) & M;                      // Eq. (6) under |dh| <= N: blocked iff a neighbour sits at h - N
+                    const bool ok = (((bL >> sn) & M) != tq) & (((bR >> sn) & M) != tq) & (((bU >> s) & M) != tq) &
+                                    (((bD >> s) & M) != tq);
+                    if (ok) fine_sts_u8(aC, (bC & ~(15u << s)) | (((c + 1u) & M) << s));
+                    return ok ? 1u : 0u;
+                };
+                if (POISSON) {
+                    // D:2c: n ~ Poisson(4) attempts from the first word of Philox call 0xFFFFFFFF of this cell
+                    const uint32_t cnt = poisson4_count(philox4x32_10(0xFFFFFFFFu, tile_id, u, rg, p.k0, p.k1).x);
+                    uint4 o = make_uint4(0, 0, 0, 0);
 #pragma unroll 1
-                for (uint32_t q = 0; q < A / 8u; ++q) {
-                    const uint4 o = philox4x32_10(q, tile_id, u, rg, p.k0, p.k1);
-                    const uint32_t ow[4] = {o.x, o.y, o.z, o.w};
+                    for (uint32_t a = 0; a < cnt; ++a) {
+                        const uint32_t w = a & 7u;
+                        if (w == 0u) o = philox4x32_10(a >> 3, tile_id, u, rg, p.k0, p.k1);
+                        const uint32_t word = (w >> 1) == 0u ? o.x : (w >> 1) == 1u ? o.y : (w >> 1) == 2u ? o.z : o.w;
+                        nacc += attempt((w & 1u) ? word >> 16 : word);
+                    }
+                } else {
+#pragma unroll 1
+                    for (uint32_t q = 0; q < A / 8u; ++q) {
+                        const uint4 o = philox4x32_10(q, tile_id, u, rg, p.k0, p.k1);
+                        const uint32_t ow[4] = {o.x, o.y, o.z, o.w};
 #pragma unroll
-                    for (uint32_t w = 0; w < 8; ++w) {                   // D:2 step 6: slot w of call q
-                        const uint32_t v = (w & 1u) ? ow[w >> 1] >> 16 : ow[w >> 1];
-                        const uint32_t x = (x0 + (v & (C - 1u))) & Lm, y = (y0 + ((v >> LGC) & (C - 1u))) & Lm;
-                        const uint32_t rowb = latb + (y << (lgL - 1u));
-                        const uint32_t aC = rowb + (x >> 1);
-                        const uint32_t bC = fine_lds_u8(aC);
-                        const uint32_t bL = fine_lds_u8(rowb + (((x - 1u) & Lm) >> 1));
-                        const uint32_t bR = fine_lds_u8(rowb + (((x + 1u) & Lm) >> 1));
-                        const uint32_t bU = fine_lds_u8(latb + (((y - 1u) & Lm) << (lgL - 1u)) + (x >> 1));
-                        const uint32_t bD = fine_lds_u8(latb + (((y + 1u) & Lm) << (lgL - 1u)) + (x >> 1));
-                        const uint32_t s = (x & 1u) * 4u, sn = 4u - s;   // my nibble; x - 1 and x + 1 sit in the other one
-                        const uint32_t c = bC >> s;
-                        const uint32_t tq = (c - N) & M;                  // Eq. (6) under |dh| <= N: blocked iff a neighbour sits at h - N
-                        const bool ok = (((bL >> sn) & M) != tq) & (((bR >> sn) & M) != tq) & (((bU >> s) & M) != tq) &
-                                        (((bD >> s) & M) != tq);
-                        if (ok) fine_sts_u8(aC, (bC & ~(15u << s)) | (((c + 1u) & M) << s));
-                        nacc += ok ? 1u : 0u;
+                        for (uint32_t w = 0; w < 8; ++w)                 // slot w of call q
+                            nacc += attempt((w & 1u) ? ow[w >> 1] >> 16 : ow[w >> 1]);
                     }
                 }
             }
@@ -159,13 +189,14 @@ static bool fine_shape(uint32_t L, uint32_t S, uint32_t R, uint32_t sm_count, Fi
 }
 
 // DT mode, cells of 8 or 16 sites, N <= 7, the 4-bit lattice of one realization within 128 KiB (L <= 512).
-bool fine_ok(uint32_t L, uint32_t N, uint32_t S, uint32_t K)
+bool fine_ok(uint32_t L, uint32_t N, uint32_t S, uint32_t K, bool poisson)
 {
     if ((S != 8 && S != 16) || N > 7 || 2 * S > L || L > 512) return false;
+    if (poisson) return K == S * S / 4;
     return (S * S) % K == 0 && S * S / K >= 8 && (S * S / K) % 8 == 0;
 }
 
-template <int LGC, int FB>
+template <int LGC, int FB, bool POISSON>
 static cudaError_t fine_t(const Params &p, uint32_t t0, uint32_t mcs, cudaStream_t st, int what, uint32_t *out)
 {
     FineShape sh;
@@ -174,15 +205,20 @@ static cudaError_t fine_t(const Params &p, uint32_t t0, uint32_t mcs, cudaStream
     const uint32_t threads = (sh.rpb * sh.cpp + 31u) / 32u * 32u;
     const uint32_t blocks = (p.R + sh.rpb - 1) / sh.rpb;
     if (what == 0) { out[0] = (uint32_t)sm; out[1] = blocks; out[2] = threads; out[3] = sh.rpb; return cudaSuccess; }
-    if (what == 1) return cudaFuncSetAttribute(fine_dt_kernel<LGC, FB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    fine_dt_kernel<LGC, FB><<<blocks, threads, sm, st>>>(p, t0, mcs, sh);
+    if (what == 1) return cudaFuncSetAttribute(fine_dt_kernel<LGC, FB, POISSON>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+    fine_dt_kernel<LGC, FB, POISSON><<<blocks, threads, sm, st>>>(p, t0, mcs, sh);
     return cudaGetLastError();
 }
 
 static cudaError_t fine_dispatch(const Params &p, uint32_t t0, uint32_t mcs, cudaStream_t st, int what, uint32_t *out)
 {
-    if (p.lgS == 3) return fine_t<3, 4>(p, t0, mcs, st, what, out);          // 8-site cells: 4-bit packed lattice (D:5)
-    if (p.lgS == 4) return p.FB == 2 ? fine_t<4, 2>(p, t0, mcs, st, what, out) : fine_t<4, 4>(p, t0, mcs, st, what, out);
+    if (p.poisson) {
+        if (p.lgS == 3) return fine_t<3, 4, true>(p, t0, mcs, st, what, out);
+        if (p.lgS == 4) return p.FB == 2 ? fine_t<4, 2, true>(p, t0, mcs, st, what, out) : fine_t<4, 4, true>(p, t0, mcs, st, what, out);
+        return cudaErrorInvalidValue;
+    }
+    if (p.lgS == 3) return fine_t<3, 4, false>(p, t0, mcs, st, what, out);   // 8-site cells: 4-bit packed lattice (D:5)
+    if (p.lgS == 4) return p.FB == 2 ? fine_t<4, 2, false>(p, t0, mcs, st, what, out) : fine_t<4, 4, false>(p, t0, mcs, st, what, out);
     return cudaErrorInvalidValue;
 }
 

@@ -40,7 +40,7 @@ uint32_t resident_blocks(const Params &p);
 cudaError_t resident_launch(const Params &p, uint32_t t0, uint32_t mcs, cudaStream_t st);
 
 // rsos_fine.cu (DT schedule with 8- or 16-site cells, thread per cell, lattice resident in shared memory)
-bool fine_ok(uint32_t L, uint32_t N, uint32_t S, uint32_t K);
+bool fine_ok(uint32_t L, uint32_t N, uint32_t S, uint32_t K, bool poisson);
 size_t fine_smem(const Params &p);
 uint32_t fine_blocks(const Params &p);
 cudaError_t fine_configure(const Params &p);

@@ -465,7 +465,9 @@ def test_dd_consistency_table_on_gpu(rsos):
     serial RS ("domain size ... noise amplitude").  Deterministic (fixed seeds); values recorded in DESIGN.md."""
     from paper_1605_02620_b200 import dd_consistency
     rows = dd_consistency.table(L=128, N=1, R=4096, seed=1, times=(1, 10, 100))
-    dev = {name: d for name, _, _, d in rows if d is not None}
+    dev = {name: d for name, _, _, d, _ in rows if d is not None}
+    eng = {name: e for name, e, _, _, _ in rows}
+    assert eng["DT(8,1)"] == eng["DT(16,1)"] == eng["DTP(8)"] == "fine"
     bias_t1 = [abs(dev["DT(%d,1)" % S][0][0]) for S in (8, 16, 32, 64)]
     assert bias_t1 == sorted(bias_t1, reverse=True) and bias_t1[0] > 0.03 > 0.006 > bias_t1[3]
     for i in range(3):                                      # the fidelity setting agrees with serial dynamics
@@ -473,6 +475,10 @@ def test_dd_consistency_table_on_gpu(rsos):
         assert abs(dw) < 4 * sdw and abs(dh) < 5e-4
     dw, sdw, _, _ = dev["DT(64,1)"][2]                      # the default: unresolvable from t ~ 100 on
     assert abs(dw) < 3 * sdw
+    for name in ("DTP(8)", "DTP(16)"):                      # the Poisson variant of the paper's small cells agrees with
+        for i in range(3):                                  # serial dynamics (S 8(c).4), where fixed counts are 1.6-3.6 % low
+            dw, sdw, dh, sdh = dev[name][i]
+            assert abs(dw) < 4.5 * sdw and abs(dh) < 4.5 * sdh, (name, i, dw, sdw, dh, sdh)
 
 
 def test_growth_exponent_sanity_c2(rsos):
@@ -602,3 +608,22 @@ def test_dt_fine_engine_saturated_restart_and_cross_engine(rsos, oracle_mod):
     compare(t, o, "thread on the same cells")
     g.close()
     t.close()
+
+
+@pytest.mark.parametrize("L,N,R,S,mcs,seed", [(64, 1, 9, 8, 5, 1), (128, 2, 40, 8, 3, 2), (256, 1, 3, 16, 3, 3),
+                                              (512, 1, 1, 8, 2, 4), (32, 7, 20, 16, 6, 5)])
+def test_dt_fine_engine_poisson_variant_equals_oracle(rsos, oracle_mod, L, N, R, S, mcs, seed):
+    """opts.poisson: DTP(c) -- K = c^2 / 4 sub-sweeps per MCS, Poisson(4) attempts per cell and
+    sub-sweep from the inversion table; FINE engine against the oracle's DTP, bit for bit."""
+    g = rsos.Rsos(L, N, R, seed, tile=S, poisson=True, first_real=3)
+    o = oracle_mod.Oracle(L, N, R, seed, tile=S, poisson=True, first_real=3)
+    info = g.info()
+    assert info["engine"] == "fine" and info["K"] == S * S // 4, info
+    for step in (1, mcs - 1):
+        g.advance(step)
+        o.advance(step)
+        compare(g, o, "DTP fine L=%d N=%d S=%d t=%d" % (L, N, S, g.t))
+    g.close()
+    for kw in (dict(tile=32), dict(tile=8, subsweeps=4), dict(tile=8, engine=rsos.ENGINE_THREAD)):
+        with pytest.raises(rsos.RsosError):
+            rsos.Rsos(64, 1, 1, 1, poisson=True, **kw)
