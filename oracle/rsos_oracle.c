@@ -115,6 +115,7 @@ typedef struct rsos_oracle {
     int      pow2;           /* L is a power of two                                          */
     uint32_t T;              /* general-L DT mode: tiles per side (even); 0 otherwise        */
     int      poisson;        /* 1 = DTP(c): Poisson(4) attempts per cell and sub-sweep (D:2c) */
+    int      multisurface;   /* 1 = MS: shared-coordinate multisurface schedule (D:2d)  */
     uint32_t lgL, lgS;
     int32_t *h;              /* R * L * L                                                    */
     int64_t *accepted;       /* R                                                            */
@@ -396,6 +397,51 @@ int rsos_oracle_set_poisson(rsos_oracle *c, int on)
     return 0;
 }
 
+/* ------------------------------------------------------------------------------------------
+ * Shared-coordinate multisurface schedule MS.  P:75: "Each single instruction
+ * multiple thread (SIMT) unit of the GPU updates 128 realizations, in which the sequence of randomly
+ * selected coordinates for update is the same.  This correlation was broken by updating only half of
+ * the selected lattice sites in each attempt."  Reading Q5 (the paper does not say which half, nor how
+ * time is counted):
+ *   - realizations are grouped by their GLOBAL index: group g = r div 128, member b = r mod 128;
+ *   - in sweep t the group draws 2 L^2 coordinates, selection a = 0 .. 2 L^2 - 1 in order, from the
+ *     coordinate stream Philox(counter (q, 0xFFFFFFFD, t, g)) with the slot layout of RS (D:2 step 6);
+ *   - member b attempts the deposit at selection a iff bit (b mod 32) of word (b div 32) of
+ *     Philox(counter (a, 0xFFFFFFFC, t, g)) is 1: an independent fair bit per member and selection, so
+ *     each surface makes L^2 attempts per MCS on average;
+ *   - whole lattice, no decomposition (2S > L), L a power of two.
+ * A realization is still a pure function of (seed, r, t): this function follows one realization alone.
+ * ------------------------------------------------------------------------------------------ */
+static void one_mcs_multisurface(rsos_oracle *c, uint32_t rl, uint64_t t)
+{
+    const uint32_t L = c->L, lgL = c->lgL;
+    int32_t *h = c->h + (size_t)rl * L * L;
+    const uint32_t rg = c->first_real + rl, g = rg >> 7, b = rg & 127u;
+    const uint32_t key[2] = { (uint32_t)(c->seed & 0xffffffffu), (uint32_t)(c->seed >> 32) };
+    const uint32_t w = (2 * lgL <= 16) ? 16 : 32, ns = 128 / w;
+    const uint64_t A = 2ull * L * L;
+    uint32_t co[4] = { 0, 0, 0, 0 };
+    int64_t acc = 0;
+    for (uint64_t a = 0; a < A; ++a) {
+        const uint32_t j = (uint32_t)(a % ns);
+        if (j == 0) { uint32_t cc[4] = { (uint32_t)(a / ns), 0xFFFFFFFDu, (uint32_t)t, g }; rsos_oracle_philox(cc, key, co); }
+        const uint32_t v = (w == 16) ? (co[j >> 1] >> (16 * (j & 1))) & 0xffffu : co[j];
+        const uint32_t x = v & (L - 1), y = (v >> lgL) & (L - 1);
+        uint32_t mc[4] = { (uint32_t)a, 0xFFFFFFFCu, (uint32_t)t, g }, mo[4];
+        rsos_oracle_philox(mc, key, mo);
+        if ((mo[b >> 5] >> (b & 31u)) & 1u) acc += attempt_checked(c, h, x, y);
+    }
+    c->accepted[rl] += acc;
+}
+
+int rsos_oracle_set_multisurface(rsos_oracle *c, int on)
+{
+    if (on && (c->mode_dt || !c->pow2 || 2ull * c->L * c->L >= (1ull << 32))) {
+        snprintf(g_err, sizeof g_err, "MS needs RS mode on a power-of-two lattice"); return -1; }
+    c->multisurface = on ? 1 : 0;
+    return 0;
+}
+
 static uint64_t splitmix64(uint64_t *s)
 { uint64_t z = (*s += 0x9E3779B97F4A7C15ull); z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
   z = (z ^ (z >> 27)) * 0x94D049BB133111EBull; return z ^ (z >> 31); }
@@ -413,6 +459,7 @@ static void one_mcs(rsos_oracle *c, uint32_t rl, uint64_t t, int par_tiles)
     int32_t *h = c->h + (size_t)rl * L * L;
     const uint32_t rg = c->first_real + rl;
     if (!c->pow2) { one_mcs_general(c, rl, t, par_tiles); return; }
+    if (c->multisurface) { one_mcs_multisurface(c, rl, t); return; }
     if (!c->mode_dt) {
         c->accepted[rl] += run_tile(c, h, rg, (uint32_t)t, 0, 0, 0, L, c->lgL, (uint64_t)L * L);
         return;

@@ -73,6 +73,8 @@ def lib():
         l.rsos_oracle_poisson4.restype = u32
         l.rsos_oracle_set_poisson.argtypes = [vp, C.c_int]
         l.rsos_oracle_set_poisson.restype = C.c_int
+        l.rsos_oracle_set_multisurface.argtypes = [vp, C.c_int]
+        l.rsos_oracle_set_multisurface.restype = C.c_int
         l.rsos_oracle_bounded.argtypes = [u32, u32, C.POINTER(C.c_int)]
         l.rsos_oracle_bounded.restype = u32
         l.rsos_oracle_bounded_census.argtypes = [u32, vp, C.POINTER(u64)]
@@ -125,7 +127,7 @@ class Oracle:
     """Same five logical operations as the C-ABI library (init / advance / width / sums / state)."""
 
     def __init__(self, L, N, R, seed, tile=64, subsweeps=1, first_real=0, threads=0,
-                 check_each=False, shuffle_seed=0, poisson=False):
+                 check_each=False, shuffle_seed=0, poisson=False, multisurface=False):
         self.L, self.N, self.R, self.seed = int(L), int(N), int(R), int(seed)
         self._l = lib()
         self._c = self._l.rsos_oracle_create(self.L, self.N, self.R, self.seed, int(tile), int(subsweeps),
@@ -135,6 +137,8 @@ class Oracle:
         self._l.rsos_oracle_set_debug(self._c, int(bool(check_each)), int(shuffle_seed), int(threads))
         if poisson and self._l.rsos_oracle_set_poisson(self._c, 1) != 0:
             raise ValueError("rsos_oracle_set_poisson: " + self._l.rsos_oracle_last_error().decode())
+        if multisurface and self._l.rsos_oracle_set_multisurface(self._c, 1) != 0:
+            raise ValueError("rsos_oracle_set_multisurface: " + self._l.rsos_oracle_last_error().decode())
 
     def close(self):
         if self._c:
