@@ -68,6 +68,9 @@ enum {
                              /* lattice sites", P:204 16 x 16): tile = 8 or 16, N <= 7, L <= 512.  One thread */
                              /* per cell works straight on a 4-bit lattice that stays in shared memory for    */
                              /* all passes of an rsos_advance call (one or more realizations per block)       */
+    RSOS_ENGINE_MULTI = 7,   /* the schedule of opts.multisurface: one warp per 32 realizations that share    */
+                             /* their coordinates, surfaces in shared memory with the realization innermost   */
+                             /* (every access coalesced and conflict-free); serial mode, L <= 32, N <= 31     */
     RSOS_ENGINE_RESIDENT = 5 /* DT mode, small lattices: a cluster of thread blocks keeps the     */
                              /* lattice of one realization in (distributed) shared memory for     */
                              /* every colour pass, sub-sweep and MCS of an rsos_advance call; one */
@@ -104,6 +107,12 @@ typedef struct rsos_opts {
                           /* shares its shared memory), 1, 2, 4, 8 or 16; must divide the (L / 2 tile)^2  */
                           /* tiles of a colour pass; 0 = chosen by the library.  Does not change the      */
                           /* result.                                                                      */
+    uint32_t multisurface;/* 1: the paper's shared-coordinate multisurface scheme (schedule MS, D:2d): groups */
+                          /* of 128 realizations (by global index) share one coordinate sequence of 2 L^2           */
+                          /* selections per MCS, and a member attempts a selection iff its own random bit is set    */
+                          /* ("updating only half of the selected lattice sites"): L^2 attempts per surface and MCS  */
+                          /* on average.  A different stochastic process from the default (surfaces of a group are  */
+                          /* correlated); serial mode (2 * tile > L), L <= 32, N <= 31, first_real % 32 == 0.        */
 } rsos_opts;
 
 /*

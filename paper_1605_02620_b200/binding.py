@@ -12,8 +12,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "librsos.so")
 
-ENGINE_AUTO, ENGINE_SIMPLE, ENGINE_WARP, ENGINE_ONCHIP, ENGINE_THREAD, ENGINE_RESIDENT, ENGINE_FINE = 0, 1, 2, 3, 4, 5, 6
-ENGINE_NAMES = {0: "auto", 1: "simple", 2: "warp", 3: "onchip", 4: "thread", 5: "resident", 6: "fine"}
+ENGINE_AUTO, ENGINE_SIMPLE, ENGINE_WARP, ENGINE_ONCHIP, ENGINE_THREAD, ENGINE_RESIDENT, ENGINE_FINE, ENGINE_MULTI = 0, 1, 2, 3, 4, 5, 6, 7
+ENGINE_NAMES = {0: "auto", 1: "simple", 2: "warp", 3: "onchip", 4: "thread", 5: "resident", 6: "fine", 7: "multi"}
 RSOS_OK, RSOS_EINVAL, RSOS_ERANGE, RSOS_ENOMEM, RSOS_ECUDA, RSOS_EUNSUP = 0, -1, -2, -3, -4, -5
 
 # every symbol include/rsos.h declares (tests check the .so exports exactly these)
@@ -25,7 +25,7 @@ SYMBOLS = ("rsos_init", "rsos_advance", "rsos_sums", "rsos_width", "rsos_moments
 class RsosOpts(C.Structure):
     _fields_ = [("tile", C.c_uint32), ("subsweeps", C.c_uint32), ("first_real", C.c_uint32),
                 ("engine", C.c_uint32), ("d_heights", C.c_void_p), ("stream", C.c_void_p),
-                ("device", C.c_int32), ("lanes", C.c_uint32), ("poisson", C.c_uint32), ("cluster", C.c_uint32)]
+                ("device", C.c_int32), ("lanes", C.c_uint32), ("poisson", C.c_uint32), ("cluster", C.c_uint32), ("multisurface", C.c_uint32)]
 
 
 class RsosError(RuntimeError):
@@ -72,9 +72,9 @@ def _check(rc):
         raise RsosError(rc, load().rsos_last_error().decode())
 
 
-def plan(L, N, R, tile=0, subsweeps=0, engine=ENGINE_AUTO, lanes=0, sm_count=0, cluster=0, poisson=False):
+def plan(L, N, R, tile=0, subsweeps=0, engine=ENGINE_AUTO, lanes=0, sm_count=0, cluster=0, poisson=False, multisurface=False):
     """rsos_plan: what rsos_init would choose for these arguments (host only, no device needed)."""
-    o = RsosOpts(int(tile), int(subsweeps), 0, int(engine), None, None, 0, int(lanes), int(bool(poisson)), int(cluster))
+    o = RsosOpts(int(tile), int(subsweeps), 0, int(engine), None, None, 0, int(lanes), int(bool(poisson)), int(cluster), int(bool(multisurface)))
     a = (C.c_uint64 * 9)()
     _check(load().rsos_plan(int(L), int(N), int(R), C.byref(o), int(sm_count), a))
     return {"mode": "DT" if a[0] else "RS", "engine": ENGINE_NAMES[a[1]], "S": a[2], "K": a[3], "pass_tiles": a[4],
@@ -99,11 +99,11 @@ class Rsos:
     """
 
     def __init__(self, L, N, R, seed, tile=0, subsweeps=0, first_real=0, engine=ENGINE_AUTO,
-                 d_heights=None, stream=None, device=None, lanes=0, cluster=0, poisson=False):
+                 d_heights=None, stream=None, device=None, lanes=0, cluster=0, poisson=False, multisurface=False):
         self._l = load()
         self.L, self.N, self.R, self.seed = int(L), int(N), int(R), int(seed)
         o = RsosOpts(int(tile), int(subsweeps), int(first_real), int(engine), d_heights or None,
-                     stream or None, 0 if device is None else int(device) + 1, int(lanes), int(bool(poisson)), int(cluster))
+                     stream or None, 0 if device is None else int(device) + 1, int(lanes), int(bool(poisson)), int(cluster), int(bool(multisurface)))
         self._c = C.c_void_p()
         _check(self._l.rsos_init(C.byref(self._c), self.L, self.N, self.R, self.seed, C.byref(o)))
 

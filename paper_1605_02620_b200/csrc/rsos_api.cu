@@ -121,10 +121,12 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
         return fail(RSOS_EINVAL, "opts.lanes = %u must be 0, 1, 2, 4 or 8", opt.lanes);
     if (opt.cluster != 0 && opt.cluster != 1 && opt.cluster != 2 && opt.cluster != 4 && opt.cluster != 8 && opt.cluster != 16)
         return fail(RSOS_EINVAL, "opts.cluster = %u must be 0, 1, 2, 4, 8 or 16", opt.cluster);
-    if (opt.engine > RSOS_ENGINE_FINE) return fail(RSOS_EINVAL, "unknown engine %u", opt.engine);
+    if (opt.engine > RSOS_ENGINE_MULTI) return fail(RSOS_EINVAL, "unknown engine %u", opt.engine);
     uint32_t S = opt.tile ? opt.tile : 64, K = opt.subsweeps ? opt.subsweeps : 1;
     if (!is_pow2(S) || S < 8) return fail(RSOS_EINVAL, "tile = %u must be a power of two >= 8", S);
     if (opt.poisson > 1) return fail(RSOS_EINVAL, "opts.poisson = %u must be 0 or 1", opt.poisson);
+    if (opt.multisurface > 1) return fail(RSOS_EINVAL, "opts.multisurface = %u must be 0 or 1", opt.multisurface);
+    if (opt.multisurface && opt.poisson) return fail(RSOS_EINVAL, "opts.multisurface and opts.poisson exclude each other");
     if (opt.poisson) {                                     // D:2c: K = tile^2 / 4 sub-sweeps of Poisson(4) attempts per cell
         if (S != 8 && S != 16) return fail(RSOS_EINVAL, "opts.poisson needs tile = 8 or 16");
         if (opt.subsweeps && opt.subsweeps != S * S / 4) return fail(RSOS_EINVAL, "opts.poisson fixes subsweeps = tile^2 / 4 = %u", S * S / 4);
@@ -155,6 +157,15 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
     if (mode_dt && !general) {
         if (opt.cluster) { if (resident_ok(L, N, S, K, opt.cluster, smem_limit)) res_cluster = opt.cluster; }
         else res_cluster = resident_cluster_size(L, N, S, K, R, sm_count, smem_limit);
+    }
+    if (opt.multisurface) {                                // D:2d: the shared-coordinate schedule MS, MULTI engine
+        if (mode_dt || general) return fail(RSOS_EINVAL, "opts.multisurface needs the serial mode (2 * tile > L) on a power-of-two lattice");
+        if (!multi_ok(L, N, opt.first_real))
+            return fail(RSOS_EUNSUP, "opts.multisurface runs on the MULTI engine: L <= 32, N <= 31, first_real a multiple of 32");
+        if (engine != RSOS_ENGINE_AUTO && engine != RSOS_ENGINE_MULTI) return fail(RSOS_EUNSUP, "opts.multisurface runs on the MULTI engine only");
+        engine = RSOS_ENGINE_MULTI;
+    } else if (engine == RSOS_ENGINE_MULTI) {
+        return fail(RSOS_EINVAL, "engine MULTI runs the schedule of opts.multisurface only");
     }
     const bool fine_can = !general && mode_dt && fine_ok(L, N, S, K, opt.poisson != 0);
     if (opt.poisson && !fine_can)
@@ -272,6 +283,7 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
     p.S = S; p.lgS = ilog2(S); p.K = K;
     p.general = pl.general ? 1u : 0u; p.T = pl.T;
     p.poisson = opt.poisson ? 1u : 0u;
+    p.multisurface = opt.multisurface ? 1u : 0u;
     p.k0 = (uint32_t)(seed & 0xFFFFFFFFull); p.k1 = (uint32_t)(seed >> 32);
 
 #define INIT_TRY(expr, code)                                                                             \
@@ -323,7 +335,7 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
     INIT_TRY(cudaEventCreate(&c->ev1), RSOS_ECUDA);
     c->smem_bytes = engine == RSOS_ENGINE_WARP ? warp_dt_smem(p.lgS) : engine == RSOS_ENGINE_ONCHIP ? warp_rs_smem(p.lgL)
                     : engine == RSOS_ENGINE_THREAD ? thread_dt_smem(p) : engine == RSOS_ENGINE_RESIDENT ? resident_smem(p)
-                    : engine == RSOS_ENGINE_FINE ? fine_smem(p) : 0;
+                    : engine == RSOS_ENGINE_FINE ? fine_smem(p) : engine == RSOS_ENGINE_MULTI ? multi_smem(p) : 0;
 #undef INIT_TRY
     *out = c;
     return RSOS_OK;
@@ -445,6 +457,12 @@ extern "C" int rsos_advance(rsos_ctx *c, uint64_t mcs)
                     ++c->launches;
                 }
             }
+    } else if (c->engine == RSOS_ENGINE_MULTI) {
+        for (uint64_t m = 0; m < mcs; m += 4096) {         // the on-chip int16 heights are good for 4096 MCS per launch
+            const uint64_t n = mcs - m < 4096 ? mcs - m : 4096;
+            CUDA_TRY(launch_rs_sweeps(p, c->engine, (uint32_t)(c->t + m), (uint32_t)n, c->blocks, c->stream));
+            ++c->launches;
+        }
     } else {
         CUDA_TRY(launch_rs_sweeps(p, c->engine, (uint32_t)c->t, (uint32_t)mcs, c->blocks, c->stream));
         ++c->launches;

@@ -48,6 +48,7 @@ struct Params {
     uint32_t FB;                    // field bits of pk (2 or 4); 0 when there is no packed lattice
     uint32_t KL;                    // THREAD engine: lanes per tile (1, 2, 4 or 8)
     uint32_t poisson;               // 1: Poisson variant DTP(c) (D:2c): Poisson(4) attempts per cell and sub-sweep
+    uint32_t multisurface;          // 1: shared-coordinate multisurface schedule MS (D:2d), MULTI engine
     uint32_t sm_count;              // SMs of the device (launch shapes)
     uint32_t general;               // 1: L is not a power of two -- general-L schedule RSG / DTG (D:2b), SIMPLE engine
     uint32_t T;                     // general DT mode: tiles per side, 2 * floor(L / 2S)

@@ -12,7 +12,7 @@ struct Params;
 constexpr int WARP_DT_WARPS = 1;     // warps (= tiles) per block of the DT warp engine (1: even spread over SMs)
 constexpr int WARP_RS_WARPS = 4;     // warps (= realizations) per block of the on-chip RS engine
 
-enum : uint32_t { ENGINE_AUTO = 0, ENGINE_SIMPLE = 1, ENGINE_WARP = 2, ENGINE_ONCHIP = 3, ENGINE_THREAD = 4, ENGINE_RESIDENT = 5, ENGINE_FINE = 6 };
+enum : uint32_t { ENGINE_AUTO = 0, ENGINE_SIMPLE = 1, ENGINE_WARP = 2, ENGINE_ONCHIP = 3, ENGINE_THREAD = 4, ENGINE_RESIDENT = 5, ENGINE_FINE = 6, ENGINE_MULTI = 7 };
 
 // rsos_update.cu
 size_t warp_dt_smem(uint32_t lgS);
@@ -45,6 +45,13 @@ size_t fine_smem(const Params &p);
 uint32_t fine_blocks(const Params &p);
 cudaError_t fine_configure(const Params &p);
 cudaError_t fine_launch(const Params &p, uint32_t t0, uint32_t mcs, cudaStream_t st);
+
+// rsos_multi.cu (shared-coordinate multisurface schedule MS, realizations innermost in shared memory)
+bool multi_ok(uint32_t L, uint32_t N, uint32_t first_real);
+size_t multi_smem(const Params &p);
+uint32_t multi_blocks(const Params &p);
+cudaError_t multi_configure(const Params &p);
+cudaError_t multi_launch(const Params &p, uint32_t t0, uint32_t mcs, cudaStream_t st);
 
 // rsos_pack.cu (packed working lattice <-> int32 heights)
 cudaError_t launch_pack(const Params &p, cudaStream_t st);

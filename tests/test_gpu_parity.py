@@ -627,3 +627,34 @@ def test_dt_fine_engine_poisson_variant_equals_oracle(rsos, oracle_mod, L, N, R,
     for kw in (dict(tile=32), dict(tile=8, subsweeps=4), dict(tile=8, engine=rsos.ENGINE_THREAD)):
         with pytest.raises(rsos.RsosError):
             rsos.Rsos(64, 1, 1, 1, poisson=True, **kw)
+
+
+@pytest.mark.parametrize("L,N,R,mcs,first", [(32, 1, 256, 6, 0), (16, 2, 70, 9, 96), (8, 31, 33, 12, 32), (32, 1, 20, 4, 224)])
+def test_multisurface_shared_coordinates_equals_oracle(rsos, oracle_mod, L, N, R, mcs, first):
+    """opts.multisurface: the paper's shared-coordinate multisurface scheme (schedule MS) on
+    the MULTI engine (realizations innermost in shared memory) against the oracle's MS, bit for bit; R spans several
+    groups of 128 and ragged warps."""
+    g = rsos.Rsos(L, N, R, 6, multisurface=True, first_real=first)
+    o = oracle_mod.Oracle(L, N, R, 6, multisurface=True, first_real=first)
+    assert g.info()["engine"] == "multi" and g.info()["mode"] == "RS"
+    for step in (1, mcs - 1):
+        g.advance(step)
+        o.advance(step)
+        compare(g, o, "MS L=%d N=%d t=%d" % (L, N, g.t))
+    g.close()
+    for kw in (dict(first_real=5), dict(tile=8), dict(engine=rsos.ENGINE_ONCHIP)):
+        with pytest.raises(rsos.RsosError):
+            rsos.Rsos(32, 1, 32, 1, multisurface=True, **kw)
+    with pytest.raises(rsos.RsosError):
+        rsos.Rsos(64, 1, 32, 1, multisurface=True)
+
+
+def test_multisurface_long_launch_chunks(rsos, oracle_mod):
+    """More than 4096 MCS in one call (the int16 on-chip heights are re-based every 4096 MCS) and a saturated surface."""
+    L, N, R = 8, 1, 32
+    g = rsos.Rsos(L, N, R, 3, multisurface=True)
+    o = oracle_mod.Oracle(L, N, R, 3, multisurface=True)
+    g.advance(9000)
+    o.advance(9000)
+    compare(g, o, "MS 9000 MCS")
+    g.close()
