@@ -328,7 +328,7 @@ def test_moments_exact(rsos, engine):
 
 
 def test_error_paths(rsos):
-    for args, kw in [((48, 1, 1, 1), {}), ((64, 0, 1, 1), {}), ((64, 1, 0, 1), {}), ((64, 200, 1, 1), {}),
+    for args, kw in [((3, 1, 1, 1), {}), ((65537, 1, 1, 1), {}), ((64, 0, 1, 1), {}), ((64, 1, 0, 1), {}), ((64, 200, 1, 1), {}),
                      ((128, 1, 1, 1), dict(tile=24)), ((128, 1, 1, 1), dict(tile=8, subsweeps=4)),
                      ((128, 1, 1, 1), dict(subsweeps=3))]:
         with pytest.raises(rsos.RsosError) as e:
