@@ -201,13 +201,34 @@ __global__ void __launch_bounds__(256) unpack_rows_kernel(const uint32_t *__rest
             mn = min(mn, __shfl_xor_sync(0xFFFFFFFFu, mn, o));
             mx = max(mx, __shfl_xor_sync(0xFFFFFFFFu, mx, o));
         }
-        if (lane == 0 && row_ok) {
-            unsigned long long *d = srel + 4 * (size_t)rl;
-            if (acc != 0) atomicAdd(d, (unsigned long long)acc);
-            if (acc2 != 0) atomicAdd(d + 1, acc2);
-            if (mn <= mx) {
-                atomicMin(reinterpret_cast<long long *>(d + 2), (long long)mn);
-                atomicMax(reinterpret_cast<long long *>(d + 3), (long long)mx);
+        // The rows of one block belong to one realization whenever a realization has at least 8 rows (L >= 8, always):
+        // team_block: one row; else 8 consecutive rows, and L is a multiple of 8.  Reduce over the 8 warps first so
+        // that a block sends ONE set of atomics (they all land on the four words of its realization).
+        __shared__ long long b_acc[8];
+        __shared__ unsigned long long b_acc2[8];
+        __shared__ int32_t b_mn[8], b_mx[8];
+        if (lane == 0) {
+            b_acc[warp] = row_ok ? acc : 0;
+            b_acc2[warp] = row_ok ? acc2 : 0ull;
+            b_mn[warp] = row_ok ? mn : 0x7FFFFFFF;
+            b_mx[warp] = row_ok ? mx : -0x7FFFFFFF - 1;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const uint32_t row0 = team_block ? blockIdx.x : blockIdx.x * 8u;
+            if (row0 < nrows) {
+                long long a = 0;
+                unsigned long long a2 = 0;
+                int32_t lo = 0x7FFFFFFF, hi = -0x7FFFFFFF - 1;
+#pragma unroll
+                for (int w = 0; w < 8; ++w) { a += b_acc[w]; a2 += b_acc2[w]; lo = min(lo, b_mn[w]); hi = max(hi, b_mx[w]); }
+                unsigned long long *d = srel + 4 * (size_t)(row0 / L);
+                if (a != 0) atomicAdd(d, (unsigned long long)a);
+                if (a2 != 0) atomicAdd(d + 1, a2);
+                if (lo <= hi) {
+                    atomicMin(reinterpret_cast<long long *>(d + 2), (long long)lo);
+                    atomicMax(reinterpret_cast<long long *>(d + 3), (long long)hi);
+                }
             }
         }
     }
