@@ -55,7 +55,7 @@ def parse():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", default="C2", help="C1..C5, or e.g. C3/N=2, C5/L=256")
     ap.add_argument("--mcs-per-step", type=int, default=0, help="MCS per step (0 = workload default)")
-    ap.add_argument("--engine", default="auto", choices=["auto", "simple", "warp", "onchip", "thread", "resident"])
+    ap.add_argument("--engine", default="auto", choices=["auto", "simple", "warp", "onchip", "thread", "resident", "fine", "level"])
     ap.add_argument("--lanes", type=int, default=0, help="THREAD engine lanes per tile (0 = auto)")
     ap.add_argument("--tile", type=int, default=0)
     ap.add_argument("--subsweeps", type=int, default=0)
@@ -413,7 +413,7 @@ def run_b200(args):
     import paper_1605_02620_b200 as pkg
 
     c = workload(args)
-    engine = {"auto": 0, "simple": 1, "warp": 2, "onchip": 3, "thread": 4, "resident": 5}[args.engine]
+    engine = {"auto": 0, "simple": 1, "warp": 2, "onchip": 3, "thread": 4, "resident": 5, "fine": 6, "level": 8}[args.engine]
     head = run_leg(pkg, torch, args.workload, c, args.steps, args.warmup, engine, args.lanes, rank, world, local, barrier,
                    not args.no_e2e, dist)
 

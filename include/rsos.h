@@ -48,8 +48,8 @@ enum {
 
 /* Update engines.  All of them produce bit-identical heights (tests/test_gpu_parity.py).       */
 enum {
-    RSOS_ENGINE_AUTO   = 0,  /* RS mode: ONCHIP when the lattice fits in shared memory, else      */
-                             /* SIMPLE.  DT mode: FINE when it applies (tile 8 or 16, L <= 512),  */
+    RSOS_ENGINE_AUTO   = 0,  /* RS mode: LEVEL for few realizations, else ONCHIP when the lattice */
+                             /* fits in shared memory, else SIMPLE.  DT mode: FINE when it applies (tile 8 or 16, L <= 512),  */
                              /* else THREAD when it applies and one colour pass has               */
                              /* at least RSOS_THREAD_MIN_TILES active tiles, else RESIDENT when   */
                              /* it applies, else WARP, else SIMPLE                                */
@@ -71,6 +71,10 @@ enum {
     RSOS_ENGINE_MULTI = 7,   /* the schedule of opts.multisurface: one warp per 32 realizations that share    */
                              /* their coordinates, surfaces in shared memory with the realization innermost   */
                              /* (every access coalesced and conflict-free); serial mode, L <= 32, N <= 31     */
+    RSOS_ENGINE_LEVEL = 8,   /* RS mode with few realizations (AUTO: R <= 2 x SM count): a block per          */
+                             /* realization keeps the lattice in shared memory and runs batches of 256        */
+                             /* consecutive attempts in dependency levels (an attempt waits only for earlier  */
+                             /* attempts at equal or adjacent sites); 16 <= L <= 128                          */
     RSOS_ENGINE_RESIDENT = 5 /* DT mode, small lattices: a cluster of thread blocks keeps the     */
                              /* lattice of one realization in (distributed) shared memory for     */
                              /* every colour pass, sub-sweep and MCS of an rsos_advance call; one */

@@ -12,8 +12,8 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "librsos.so")
 
-ENGINE_AUTO, ENGINE_SIMPLE, ENGINE_WARP, ENGINE_ONCHIP, ENGINE_THREAD, ENGINE_RESIDENT, ENGINE_FINE, ENGINE_MULTI = 0, 1, 2, 3, 4, 5, 6, 7
-ENGINE_NAMES = {0: "auto", 1: "simple", 2: "warp", 3: "onchip", 4: "thread", 5: "resident", 6: "fine", 7: "multi"}
+ENGINE_AUTO, ENGINE_SIMPLE, ENGINE_WARP, ENGINE_ONCHIP, ENGINE_THREAD, ENGINE_RESIDENT, ENGINE_FINE, ENGINE_MULTI, ENGINE_LEVEL = 0, 1, 2, 3, 4, 5, 6, 7, 8
+ENGINE_NAMES = {0: "auto", 1: "simple", 2: "warp", 3: "onchip", 4: "thread", 5: "resident", 6: "fine", 7: "multi", 8: "level"}
 RSOS_OK, RSOS_EINVAL, RSOS_ERANGE, RSOS_ENOMEM, RSOS_ECUDA, RSOS_EUNSUP = 0, -1, -2, -3, -4, -5
 
 # every symbol include/rsos.h declares (tests check the .so exports exactly these)

@@ -121,7 +121,7 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
         return fail(RSOS_EINVAL, "opts.lanes = %u must be 0, 1, 2, 4 or 8", opt.lanes);
     if (opt.cluster != 0 && opt.cluster != 1 && opt.cluster != 2 && opt.cluster != 4 && opt.cluster != 8 && opt.cluster != 16)
         return fail(RSOS_EINVAL, "opts.cluster = %u must be 0, 1, 2, 4, 8 or 16", opt.cluster);
-    if (opt.engine > RSOS_ENGINE_MULTI) return fail(RSOS_EINVAL, "unknown engine %u", opt.engine);
+    if (opt.engine > RSOS_ENGINE_LEVEL) return fail(RSOS_EINVAL, "unknown engine %u", opt.engine);
     uint32_t S = opt.tile ? opt.tile : 64, K = opt.subsweeps ? opt.subsweeps : 1;
     if (!is_pow2(S) || S < 8) return fail(RSOS_EINVAL, "tile = %u must be a power of two >= 8", S);
     if (opt.poisson > 1) return fail(RSOS_EINVAL, "opts.poisson = %u must be 0 or 1", opt.poisson);
@@ -172,8 +172,12 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
         return fail(RSOS_EUNSUP, "opts.poisson runs on the FINE engine: L <= 512 (a power of two) and N <= 7");
     if (opt.poisson && engine != RSOS_ENGINE_AUTO && engine != RSOS_ENGINE_FINE)
         return fail(RSOS_EUNSUP, "opts.poisson runs on the FINE engine only");
+    const bool level_can = !general && !mode_dt && !opt.multisurface && level_ok(L, N);
     if (engine == RSOS_ENGINE_AUTO) {
-        if (!mode_dt) engine = onchip_ok ? RSOS_ENGINE_ONCHIP : RSOS_ENGINE_SIMPLE;
+        // serial RS: a warp per realization (ONCHIP) when there are enough realizations to fill the machine, else a
+        // block per realization that runs a batch of attempts in dependency levels (LEVEL)
+        if (!mode_dt) engine = (level_can && R <= 2u * (uint32_t)sm_count) ? RSOS_ENGINE_LEVEL
+                               : onchip_ok ? RSOS_ENGINE_ONCHIP : level_can ? RSOS_ENGINE_LEVEL : RSOS_ENGINE_SIMPLE;
         else if (fine_can) engine = RSOS_ENGINE_FINE;                  // 8- or 16-site cells on a lattice that fits on chip
         else if (thread_ok && pass_tiles >= RSOS_THREAD_MIN_TILES) engine = RSOS_ENGINE_THREAD;
         else if (res_cluster && pass_tiles / R <= 16) engine = RSOS_ENGINE_RESIDENT;   // few tiles per pass and realization
@@ -184,6 +188,8 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
                                  "the (L / 2 tile)^2 tiles of a colour pass with at most 16 tiles per block, and the lattice slab in shared memory");
     if (engine == RSOS_ENGINE_FINE && !fine_can)
         return fail(RSOS_EUNSUP, "engine FINE needs DT mode with tile 8 or 16, N <= 7 and L <= 512 (the 4-bit lattice within 128 KiB)");
+    if (engine == RSOS_ENGINE_LEVEL && !level_can)
+        return fail(RSOS_EUNSUP, "engine LEVEL needs the serial mode (2 * tile > L), 16 <= L <= 128 (a power of two)");
     if (engine == RSOS_ENGINE_WARP && !warp_ok)
         return fail(RSOS_EUNSUP, "engine WARP needs DT mode (2*tile <= L), tile <= 128 and N <= 31");
     if (engine == RSOS_ENGINE_THREAD && !thread_ok)
@@ -335,7 +341,8 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
     INIT_TRY(cudaEventCreate(&c->ev1), RSOS_ECUDA);
     c->smem_bytes = engine == RSOS_ENGINE_WARP ? warp_dt_smem(p.lgS) : engine == RSOS_ENGINE_ONCHIP ? warp_rs_smem(p.lgL)
                     : engine == RSOS_ENGINE_THREAD ? thread_dt_smem(p) : engine == RSOS_ENGINE_RESIDENT ? resident_smem(p)
-                    : engine == RSOS_ENGINE_FINE ? fine_smem(p) : engine == RSOS_ENGINE_MULTI ? multi_smem(p) : 0;
+                    : engine == RSOS_ENGINE_FINE ? fine_smem(p) : engine == RSOS_ENGINE_MULTI ? multi_smem(p)
+                    : engine == RSOS_ENGINE_LEVEL ? level_smem(p) : 0;
 #undef INIT_TRY
     *out = c;
     return RSOS_OK;

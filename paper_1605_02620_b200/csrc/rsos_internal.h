@@ -12,7 +12,7 @@ struct Params;
 constexpr int WARP_DT_WARPS = 1;     // warps (= tiles) per block of the DT warp engine (1: even spread over SMs)
 constexpr int WARP_RS_WARPS = 4;     // warps (= realizations) per block of the on-chip RS engine
 
-enum : uint32_t { ENGINE_AUTO = 0, ENGINE_SIMPLE = 1, ENGINE_WARP = 2, ENGINE_ONCHIP = 3, ENGINE_THREAD = 4, ENGINE_RESIDENT = 5, ENGINE_FINE = 6, ENGINE_MULTI = 7 };
+enum : uint32_t { ENGINE_AUTO = 0, ENGINE_SIMPLE = 1, ENGINE_WARP = 2, ENGINE_ONCHIP = 3, ENGINE_THREAD = 4, ENGINE_RESIDENT = 5, ENGINE_FINE = 6, ENGINE_MULTI = 7, ENGINE_LEVEL = 8 };
 
 // rsos_update.cu
 size_t warp_dt_smem(uint32_t lgS);
@@ -52,6 +52,13 @@ size_t multi_smem(const Params &p);
 uint32_t multi_blocks(const Params &p);
 cudaError_t multi_configure(const Params &p);
 cudaError_t multi_launch(const Params &p, uint32_t t0, uint32_t mcs, cudaStream_t st);
+
+// rsos_level.cu (serial RS of few realizations: a block per realization, a batch of attempts run in dependency levels)
+bool level_ok(uint32_t L, uint32_t N);
+size_t level_smem(const Params &p);
+uint32_t level_blocks(const Params &p);
+cudaError_t level_configure(const Params &p);
+cudaError_t level_launch(const Params &p, uint32_t t0, uint32_t mcs, cudaStream_t st);
 
 // rsos_pack.cu (packed working lattice <-> int32 heights)
 cudaError_t launch_pack(const Params &p, cudaStream_t st);

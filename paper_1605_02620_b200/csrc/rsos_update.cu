@@ -547,6 +547,7 @@ cudaError_t configure_engine(const Params &p, uint32_t engine, bool mode_dt)
     if (engine == ENGINE_RESIDENT && mode_dt) return resident_configure(p);
     if (engine == ENGINE_FINE && mode_dt) return fine_configure(p);
     if (engine == ENGINE_MULTI && !mode_dt) return multi_configure(p);
+    if (engine == ENGINE_LEVEL && !mode_dt) return level_configure(p);
     if (engine == ENGINE_WARP && mode_dt) return dispatch_warp_dt(p, 0, 0, 0, nullptr, true);
     if (engine == ENGINE_ONCHIP && !mode_dt) return dispatch_warp_rs(p, 0, 0, 0, nullptr, true);
     return cudaSuccess;
@@ -560,6 +561,7 @@ uint32_t engine_blocks(const Params &p, uint32_t engine, bool mode_dt)
     if (engine == ENGINE_RESIDENT) return resident_blocks(p);
     if (engine == ENGINE_FINE) return fine_blocks(p);
     if (engine == ENGINE_MULTI) return multi_blocks(p);
+    if (engine == ENGINE_LEVEL) return level_blocks(p);
     if (engine == ENGINE_WARP) return (uint32_t)((tiles + WARP_DT_WARPS - 1) / WARP_DT_WARPS);
     if (engine == ENGINE_ONCHIP) return (uint32_t)((tiles + WARP_RS_WARPS - 1) / WARP_RS_WARPS);
     return (uint32_t)((tiles + (mode_dt ? 127 : 31)) / (mode_dt ? 128 : 32));
@@ -579,6 +581,7 @@ cudaError_t launch_rs_sweeps(const Params &p, uint32_t engine, uint32_t t0, uint
 {
     if (engine == ENGINE_ONCHIP) return dispatch_warp_rs(p, t0, mcs, blocks, st, false);
     if (engine == ENGINE_MULTI) return multi_launch(p, t0, mcs, st);
+    if (engine == ENGINE_LEVEL) return level_launch(p, t0, mcs, st);
     simple_rs_kernel<<<blocks, 32, 0, st>>>(p, t0, mcs);
     return cudaGetLastError();
 }

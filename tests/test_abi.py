@@ -91,7 +91,8 @@ def test_plan_picks_engines_lanes_and_site_width(lib_path):
     from paper_1605_02620_b200.utils import workloads as w
     c = w.CONFIGS
     p = m.plan(c["C1"]["L"], 1, c["C1"]["R"])
-    assert (p["mode"], p["engine"], p["S"], p["K"], p["launches_per_mcs"]) == ("RS", "onchip", 32, 1, 1)
+    assert (p["mode"], p["engine"], p["S"], p["K"], p["launches_per_mcs"]) == ("RS", "level", 32, 1, 1)   # 128 chains: few realizations
+    assert m.plan(32, 1, 4096)["engine"] == "onchip"                                  # many realizations: a warp each
     p = m.plan(c["C2"]["L"], 1, c["C2"]["R"])
     assert (p["mode"], p["engine"], p["pass_tiles"], p["lanes"], p["packed_bits"]) == ("DT", "thread", 8192, 4, 2)
     p = m.plan(c["C3"]["L"], 1, c["C3"]["R"])

@@ -49,10 +49,11 @@ def test_philox_device_equals_oracle(rsos, oracle_mod):
         assert (out[i] == oracle_mod.philox(ctr[i], key[i])).all()
 
 
-@pytest.mark.parametrize("engine", ["onchip", "simple"])
+@pytest.mark.parametrize("engine", ["auto", "onchip", "simple"])
 def test_c1_full_config_every_mcs(rsos, oracle_mod, engine):
-    """BASELINE.json configs[0]: L=32, N=1, R=128, 100 MCS, seed 1, sums at every MCS (tier A)."""
-    eng = {"onchip": rsos.ENGINE_ONCHIP, "simple": rsos.ENGINE_SIMPLE}[engine]
+    """BASELINE.json configs[0]: L=32, N=1, R=128, 100 MCS, seed 1, sums at every MCS (tier A).  engine = auto is the
+    LEVEL engine (few realizations), the launch configuration bench.py times."""
+    eng = {"auto": rsos.ENGINE_AUTO, "onchip": rsos.ENGINE_ONCHIP, "simple": rsos.ENGINE_SIMPLE}[engine]
     g = rsos.Rsos(32, 1, 128, 1, engine=eng)
     o = oracle_mod.Oracle(32, 1, 128, 1)
     assert g.info()["mode"] == "RS" and o.mode == "RS"
@@ -657,4 +658,22 @@ def test_multisurface_long_launch_chunks(rsos, oracle_mod):
     g.advance(9000)
     o.advance(9000)
     compare(g, o, "MS 9000 MCS")
+    g.close()
+
+
+@pytest.mark.parametrize("L,N,R,mcs,seed", [(16, 1, 3, 40, 1), (32, 2, 5, 25, 2), (64, 1, 2, 12, 3), (128, 3, 1, 5, 4),
+                                            (32, 31, 2, 20, 5), (64, 127, 1, 6, 6)])
+def test_rs_level_engine_equals_oracle(rsos, oracle_mod, L, N, R, mcs, seed):
+    """The LEVEL engine (rsos_level.cu): serial RS, a block per realization, batches of 256 attempts executed in
+    dependency levels -- the sequential result, bit for bit; several MCS per launch; heights far from the flat start."""
+    g = rsos.Rsos(L, N, R, seed, tile=L, engine=rsos.ENGINE_LEVEL, first_real=2)
+    o = oracle_mod.Oracle(L, N, R, seed, tile=L, first_real=2)
+    assert g.info()["engine"] == "level" and g.info()["mode"] == "RS"
+    for step in (1, 1, mcs - 2):
+        g.advance(step)
+        o.advance(step)
+        compare(g, o, "RS level L=%d N=%d t=%d" % (L, N, g.t))
+    g.advance(700)                                           # |h| beyond one byte: the mod-256 heights wrap
+    o.advance(700)
+    compare(g, o, "RS level late")
     g.close()
