@@ -104,6 +104,155 @@ __device__ __forceinline__ void general_dt_pass(const Params &p, uint32_t u, uin
     if (nacc) atomicAdd(p.accepted + rl, (unsigned long long)nacc);
 }
 
+// ---------------------------------------------------------------------------------------------
+// General-L DT pass with tile windows in shared memory (D:2b, N <= 7).  A warp owns GW_NT = 16 tiles: the 32 lanes
+// stage the (w + 2) x (hgt + 2) windows one tile after the other (coalesced int32 rows -> one byte per site, the
+// height mod 256), lane g < 16 then runs the attempts of tile g in order on its window, and the warp writes the
+// interiors back as h += (new byte - old byte) mod 256.  Word j of tile g lives at smem[j * 16 + g], so the 16
+// working lanes never share a bank.  Exact: Eq. (6) needs only differences (|dh| <= N < 128 survives mod 256), and
+// for N <= 7 no site can gain 256 within one pass (raising one site by 256 forces >= 256 + 4*242 + 8*228 + ... more
+// than the (2S)^2 attempts a tile has), so the byte delta is the true one.
+// ---------------------------------------------------------------------------------------------
+constexpr uint32_t GW_NT = 16;
+
+__global__ void __launch_bounds__(32) general_window_kernel(Params p, uint32_t u, uint32_t colour, uint32_t pww, uint32_t nrows)
+{
+    extern __shared__ __align__(16) uint32_t gsm[];
+    uint8_t *win = reinterpret_cast<uint8_t *>(gsm);
+    const uint32_t lane = threadIdx.x;
+    const uint32_t L = p.L, T = p.T, half = T >> 1, ntile = half * half;
+    const uint32_t total = p.R * ntile;
+    const uint32_t thrL = pow32_mod(L);
+    (void)nrows;
+
+    // geometry of tile slot g of this warp (uniform over the lanes that ask for the same g)
+    struct Tile { uint32_t rl, x0, y0, w, hgt, id, rg; bool live; };
+    auto tile_of = [&](uint32_t g) -> Tile {
+        Tile t;
+        const uint32_t idx = blockIdx.x * GW_NT + g;
+        t.live = idx < total;
+        const uint32_t i = t.live ? idx : 0u;
+        t.rl = i / ntile;
+        const uint32_t n = i - t.rl * ntile;
+        const uint32_t I = 2 * (n % half) + (colour & 1u), J = 2 * (n / half) + (colour >> 1);
+        t.rg = p.first_real + t.rl;
+        WordStream os(p, 0xFFFFFFFFu, u, t.rg);
+        const uint32_t ox = os.draw(L, thrL);
+        const uint32_t oy = os.draw(L, thrL);
+        const uint32_t bx = tile_edge(I, L, T), by = tile_edge(J, L, T);
+        t.w = tile_edge(I + 1, L, T) - bx;
+        t.hgt = tile_edge(J + 1, L, T) - by;
+        t.x0 = (ox + bx) % L;
+        t.y0 = (oy + by) % L;
+        t.id = J * T + I;
+        return t;
+    };
+    // byte address of window site (col, row) of tile g; col, row = 0 is the halo
+    auto waddr = [&](uint32_t g, uint32_t col, uint32_t row) -> uint32_t {
+        return (((row * pww + (col >> 2)) * GW_NT + g) << 2) + (col & 3u);
+    };
+
+    // ---- a3: stage.  Four rows x up to four column chunks of loads are issued before the first byte is stored, so a
+    // dozen global loads are in flight per lane (a lone warp hides no latency otherwise).
+    auto wrap3 = [&](uint32_t v) -> uint32_t { return v - ((v >= 2u * L) ? 2u * L : (v >= L ? L : 0u)); };
+    for (uint32_t g = 0; g < GW_NT; ++g) {
+        const Tile t = tile_of(g);
+        if (!t.live) break;                                              // tiles are assigned in order: the rest is idle too
+        const int32_t *h = p.h + (size_t)t.rl * L * L;
+        const uint32_t ncol = t.w + 2u, nrow = t.hgt + 2u;
+        for (uint32_t row0 = 0; row0 < nrow; row0 += 4u) {
+            int32_t v[4][4];
+#pragma unroll
+            for (uint32_t dr = 0; dr < 4; ++dr) {
+                const uint32_t row = row0 + dr < nrow ? row0 + dr : nrow - 1u;
+                const int32_t *src = h + (size_t)wrap3(t.y0 + L - 1u + row) * L;
+#pragma unroll
+                for (uint32_t dc = 0; dc < 4; ++dc) {
+                    const uint32_t col = lane + 32u * dc;
+                    v[dr][dc] = col < ncol ? src[wrap3(t.x0 + L - 1u + col)] : 0;
+                }
+            }
+#pragma unroll
+            for (uint32_t dr = 0; dr < 4; ++dr)
+#pragma unroll
+                for (uint32_t dc = 0; dc < 4; ++dc) {
+                    const uint32_t col = lane + 32u * dc;
+                    if (row0 + dr < nrow && col < ncol) win[waddr(g, col, row0 + dr)] = (uint8_t)((uint32_t)v[dr][dc] & 0xFFu);
+                }
+        }
+    }
+    __syncwarp();
+
+    // ---- a1 + a4: lane g runs tile g ----------------------------------------------------------------------------------
+    uint32_t nacc = 0;
+    Tile me = tile_of(lane < GW_NT ? lane : 0u);
+    if (lane < GW_NT && me.live) {
+        const uint32_t n = me.w * me.hgt, thr = pow32_mod(n);
+        const uint64_t k = u & (p.K - 1u);
+        const uint64_t A = ((k + 1) * (uint64_t)n) / p.K - (k * (uint64_t)n) / p.K;
+        const int32_t N = (int32_t)p.N;
+        WordStream ws(p, me.id, u, me.rg);
+        const uint32_t inv_w = 0xFFFFFFFFu / me.w;                      // s / w = mulhi(s, inv_w) or one more (s < 2^15)
+        for (uint64_t a = 0; a < A; ++a) {
+            const uint32_t s = ws.draw(n, thr);
+            uint32_t dy = __umulhi(s, inv_w);
+            uint32_t dx = s - dy * me.w;
+            if (dx >= me.w) { dx -= me.w; ++dy; }
+            const uint32_t aC = waddr(lane, dx + 1u, dy + 1u);
+            const uint32_t c = (uint32_t)win[aC] + 1u;
+            const uint32_t l = win[waddr(lane, dx, dy + 1u)], r = win[waddr(lane, dx + 2u, dy + 1u)];
+            const uint32_t up = win[aC - pww * GW_NT * 4u], dn = win[aC + pww * GW_NT * 4u];
+            auto far = [&](uint32_t nb) -> bool { return abs((int32_t)(int8_t)((c - nb) & 0xFFu)) > N; };
+            if (!(far(l) | far(r) | far(up) | far(dn))) { win[aC] = (uint8_t)c; ++nacc; }
+        }
+    }
+    __syncwarp();
+
+    // ---- a5: write back the interiors (same blocking: 4 rows x 4 column chunks of loads in flight) --------------------------
+    for (uint32_t g = 0; g < GW_NT; ++g) {
+        const Tile t = tile_of(g);
+        if (!t.live) break;
+        int32_t *h = p.h + (size_t)t.rl * L * L;
+        for (uint32_t row0 = 1; row0 <= t.hgt; row0 += 4u) {
+            int32_t old[4][4];
+            int32_t *dst[4][4];
+#pragma unroll
+            for (uint32_t dr = 0; dr < 4; ++dr) {
+                const uint32_t row = row0 + dr <= t.hgt ? row0 + dr : t.hgt;
+                int32_t *rowp = h + (size_t)wrap3(t.y0 + row - 1u) * L;
+#pragma unroll
+                for (uint32_t dc = 0; dc < 4; ++dc) {
+                    const uint32_t col = 1u + lane + 32u * dc;
+                    dst[dr][dc] = rowp + wrap3(t.x0 + (col <= t.w ? col : 1u) - 1u);
+                    old[dr][dc] = (row0 + dr <= t.hgt && col <= t.w) ? *dst[dr][dc] : 0;
+                }
+            }
+#pragma unroll
+            for (uint32_t dr = 0; dr < 4; ++dr)
+#pragma unroll
+                for (uint32_t dc = 0; dc < 4; ++dc) {
+                    const uint32_t col = 1u + lane + 32u * dc;
+                    if (row0 + dr <= t.hgt && col <= t.w) {
+                        const uint32_t d = ((uint32_t)win[waddr(g, col, row0 + dr)] - (uint32_t)old[dr][dc]) & 0xFFu;
+                        if (d) *dst[dr][dc] = old[dr][dc] + (int32_t)d;
+                    }
+                }
+        }
+    }
+    if (lane < GW_NT && me.live && nacc) atomicAdd(p.accepted + me.rl, (unsigned long long)nacc);
+}
+
+// window geometry of the general-L pass: words per window row and rows; 0 if the windows of 16 tiles do not fit
+static bool general_window_shape(const Params &p, uint32_t *pww, uint32_t *nrows, size_t *smem)
+{
+    if (!p.general || !p.T || p.N > 7) return false;
+    const uint32_t wmax = (p.L + p.T - 1) / p.T;                       // ceil(L / T): the larger of the two tile sizes
+    *pww = (wmax + 2 + 3) / 4;
+    *nrows = wmax + 2;
+    *smem = (size_t)*pww * *nrows * GW_NT * 4;
+    return *smem <= 200u * 1024u;
+}
+
 __global__ void __launch_bounds__(128) simple_dt_kernel(Params p, uint32_t u, uint32_t colour)
 {
     if (p.general) { general_dt_pass(p, u, colour, blockIdx.x * blockDim.x + threadIdx.x); return; }
@@ -550,6 +699,10 @@ cudaError_t configure_engine(const Params &p, uint32_t engine, bool mode_dt)
     if (engine == ENGINE_LEVEL && !mode_dt) return level_configure(p);
     if (engine == ENGINE_WARP && mode_dt) return dispatch_warp_dt(p, 0, 0, 0, nullptr, true);
     if (engine == ENGINE_ONCHIP && !mode_dt) return dispatch_warp_rs(p, 0, 0, 0, nullptr, true);
+    uint32_t pww, nrows;
+    size_t gsmem;
+    if (engine == ENGINE_SIMPLE && mode_dt && general_window_shape(p, &pww, &nrows, &gsmem))
+        return cudaFuncSetAttribute(general_window_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsmem);
     return cudaSuccess;
 }
 
@@ -572,6 +725,14 @@ cudaError_t launch_dt_pass(const Params &p, uint32_t engine, uint32_t u, uint32_
 {
     if (engine == ENGINE_THREAD) return thread_dt_launch(p, u, colour, blocks, st);
     if (engine == ENGINE_WARP) return dispatch_warp_dt(p, u, colour, blocks, st, false);
+    uint32_t pww, nrows;
+    size_t gsmem;
+    if (general_window_shape(p, &pww, &nrows, &gsmem)) {               // general L, N <= 7: tile windows in shared memory
+        const uint32_t half = p.T >> 1;
+        const uint64_t tiles = (uint64_t)p.R * half * half;
+        general_window_kernel<<<(uint32_t)((tiles + GW_NT - 1) / GW_NT), 32, gsmem, st>>>(p, u, colour, pww, nrows);
+        return cudaGetLastError();
+    }
     simple_dt_kernel<<<blocks, 128, 0, st>>>(p, u, colour);
     return cudaGetLastError();
 }

@@ -32,6 +32,9 @@ def _same(g, o, R):
     (200, 2, 2, 32, 4, 4, 5),        # DTG, T = 6, widths 33 / 34, four sub-sweeps of unequal attempt counts
     (100, 1, 2, 8, 2, 3, 0),         # DTG, T = 12
     (333, 3, 1, 16, 1, 2, 1),        # DTG, T = 20, odd L: scalar reductions
+    (150, 9, 2, 64, 1, 3, 0),        # N > 7: thread per tile in global memory (the windowed kernel needs N <= 7)
+    (1000, 7, 35, 64, 2, 2, 3),      # T = 14: 49 tiles per pass and realization, ragged last warp of 16 tiles, N = 7
+    (300, 1, 2, 128, 1, 2, 0),       # T = 2, tiles of 150 x 150: windows too large for shared memory -> global path
     (45, 1, 4, 64, 1, 12, 0),        # RSG (2S > L), odd L
     (6, 1, 5, 64, 1, 40, 2),         # RSG, tiny
 ])
