@@ -125,7 +125,7 @@ typedef struct rsos_opts {
  *   L     lattice side, 4 <= L <= 65536 (periodic in both directions, reading Q2).  Powers of two run the
  *         schedule D:2 on every engine; any other L (the paper's L = 9605) runs the general-L schedule
  *         D:2b -- tiles of two sizes that divide the lattice, sites drawn by an exactly uniform bounded
- *         draw -- on the SIMPLE engine only (int32 heights in global memory)
+ *         draw -- on the SIMPLE engine only (int32 heights; byte tile windows in shared memory when N <= 7)
  *   N     height-difference bound of Eq. (6), 1 <= N <= 127
  *   R     number of independent realizations, >= 1, R*L*L*4 bytes must fit on the device
  *   seed  Philox key (low word, high word)
