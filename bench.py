@@ -425,7 +425,7 @@ def run_b200(args):
                 continue
             ce = leg_config(name)
             leg = run_leg(pkg, torch, name, ce, args.extra_steps, 3, 0, 0, rank, world, local, barrier,
-                          not args.no_e2e and name in ("C4",), dist)
+                          not args.no_e2e, dist)
             leg["config"] = config_dict_for(name, ce, 1, leg["engine"])
             extra[name] = leg
 
