@@ -48,11 +48,13 @@ enum {
 
 /* Update engines.  All of them produce bit-identical heights (tests/test_gpu_parity.py).       */
 enum {
-    RSOS_ENGINE_AUTO   = 0,  /* RS mode: LEVEL for few realizations, else ONCHIP when the lattice */
-                             /* fits in shared memory, else SIMPLE.  DT mode: FINE when it applies (tile 8 or 16, L <= 512),  */
-                             /* else THREAD when it applies and one colour pass has               */
-                             /* at least RSOS_THREAD_MIN_TILES active tiles, else RESIDENT when   */
-                             /* it applies, else WARP, else SIMPLE                                */
+    RSOS_ENGINE_AUTO   = 0,  /* RS mode: LEVEL for few realizations (R <= 2 x SM count), else     */
+                             /* ONCHIP when the lattice fits in shared memory, else SIMPLE.       */
+                             /* DT mode: FINE when it applies (tile 8 or 16, L <= 512), else      */
+                             /* THREAD when it applies and one colour pass has at least           */
+                             /* RSOS_THREAD_MIN_TILES active tiles, else RESIDENT when it         */
+                             /* applies, else WARP, else SIMPLE.  L not a power of two: SIMPLE.   */
+                             /* rsos_plan() tells what a given set of arguments selects.          */
     RSOS_ENGINE_SIMPLE = 1,  /* one thread per active tile, heights in global memory (slow;       */
                              /* the literal loop nest of D:2, kept as an on-device cross-check;   */
                              /* also the engine of the general-L schedule D:2b)                   */
@@ -72,7 +74,7 @@ enum {
                              /* their coordinates, surfaces in shared memory with the realization innermost   */
                              /* (every access coalesced and conflict-free); serial mode, L <= 32, N <= 31     */
     RSOS_ENGINE_LEVEL = 8,   /* RS mode with few realizations (AUTO: R <= 2 x SM count): a block per          */
-                             /* realization keeps the lattice in shared memory and runs batches of 256        */
+                             /* realization keeps the lattice in shared memory and runs batches of 512        */
                              /* consecutive attempts in dependency levels (an attempt waits only for earlier  */
                              /* attempts at equal or adjacent sites); 16 <= L <= 128                          */
     RSOS_ENGINE_RESIDENT = 5 /* DT mode, small lattices: a cluster of thread blocks keeps the     */
@@ -94,9 +96,9 @@ typedef struct rsos_opts {
     int32_t *d_heights;   /* DEVICE: borrowed buffer of R*L*L int32 (h[r][y][x], row-major, 16-   */
                           /* byte aligned), e.g. a torch tensor; NULL = the library allocates.    */
                           /* Its content on entry is ignored: rsos_init zeroes it (flat start).   */
-                          /* With the THREAD engine the working state is a packed lattice (D:5)   */
-                          /* and this buffer is brought up to date only by rsos_get_heights,      */
-                          /* rsos_moments, rsos_set_state and rsos_device_heights.                */
+                          /* With the THREAD, RESIDENT and FINE engines the working state is a    */
+                          /* packed lattice (D:5) and this buffer is brought up to date only by   */
+                          /* rsos_get_heights, rsos_moments, rsos_set_state, rsos_device_heights. */
     void    *stream;      /* cudaStream_t to enqueue on; NULL = the legacy default stream         */
     int32_t  device;      /* CUDA device ordinal + 1; 0 = the current device                      */
     uint32_t lanes;       /* THREAD engine: lanes that share one tile, 1, 2, 4 or 8 (8 * lanes must not   */
