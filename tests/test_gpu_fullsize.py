@@ -214,3 +214,54 @@ def test_invalid_state_blocks_the_context(rsos):
         g.advance(1)
         assert (g.sums()[0] == g.sums()[2]).all()
         g.close()
+
+
+@pytest.mark.parametrize("L,S,poisson", [(64, 8, False), (128, 8, False), (256, 16, False), (512, 8, False), (128, 8, True)])
+def test_paper_cells_full_ensemble_sampled(rsos, oracle_mod, L, S, poisson):
+    """The paper's steady-state setting (8 x 8 domains, L = 64 ... 512; 16 x 16) with BASELINE configs[4]'s
+    ensemble sizes on the FINE engine (and its Poisson variant): three realizations of the full ensemble followed alone
+    by the oracle for 4 MCS; then a saturated snapshot of two of them handed to the oracle."""
+    R = workloads.c5_realizations(L)
+    kw = dict(tile=S, poisson=True) if poisson else dict(tile=S, subsweeps=1)
+    g = rsos.Rsos(L, 1, R, 1, **kw)
+    assert g.info()["engine"] == "fine"
+    g.advance(4)
+    gs = g.sums()
+    for r in (0, R // 2 + 1, R - 1):
+        o = oracle_mod.Oracle(L, 1, 1, 1, first_real=r, **kw)
+        o.advance(4)
+        os1, os2, oacc = o.sums()
+        assert (gs[0][r], gs[1][r], gs[2][r]) == (os1[0], os2[0], oacc[0])
+        assert np.array_equal(g.heights(r, 1), o.heights())
+        o.close()
+    t0 = 4 + 600
+    g.advance(600)
+    for r in (1, R - 2):
+        h, acc = g.heights(r, 1), g.sums()[2][r:r + 1]
+        o = oracle_mod.Oracle(L, 1, 1, 1, first_real=r, **kw)
+        o.set_state(h, t0, acc)
+        o.advance(1)
+        g2 = rsos.Rsos(L, 1, 1, 1, first_real=r, **kw)
+        g2.set_state(h, t0, acc)
+        g2.advance(1)
+        assert np.array_equal(g2.heights(), o.heights()) and (g2.sums()[0] == o.sums()[0]).all()
+        g2.close()
+        o.close()
+    g.close()
+
+
+def test_multisurface_large_ensemble_sampled(rsos, oracle_mod):
+    """opts.multisurface at L = 32 with 4096 realizations (32 groups of 128): members of different groups and warps
+    followed alone by the oracle (a member is a pure function of its global index) for 5 MCS."""
+    L, R = 32, 4096
+    g = rsos.Rsos(L, 1, R, 2, multisurface=True)
+    g.advance(5)
+    gs = g.sums()
+    for r in (0, 31, 32, 127, 128, 2049, 4095):
+        o = oracle_mod.Oracle(L, 1, 1, 2, first_real=r, multisurface=True)
+        o.advance(5)
+        os1, os2, oacc = o.sums()
+        assert (gs[0][r], gs[1][r], gs[2][r]) == (os1[0], os2[0], oacc[0]), r
+        assert np.array_equal(g.heights(r, 1), o.heights()), r
+        o.close()
+    g.close()

@@ -677,3 +677,47 @@ def test_rs_level_engine_equals_oracle(rsos, oracle_mod, L, N, R, mcs, seed):
     o.advance(700)
     compare(g, o, "RS level late")
     g.close()
+
+
+def test_random_shapes_new_engines(rsos, oracle_mod):
+    """Seeded random sweep over the engines added in round 2 (FINE and its Poisson variant, LEVEL, general L, MULTI):
+    random L, N, R, tile, K, first_real; heights, sums and doubles against the oracle."""
+    rng = np.random.default_rng(20261105)
+    cases = []
+    for _ in range(8):                                                   # FINE
+        S = int(rng.choice([8, 16]))
+        L = int(rng.choice([l for l in (16, 32, 64, 128, 256) if l >= 2 * S]))
+        K = int(rng.choice([k for k in (1, 2, 4, 8) if S * S // k >= 32]))
+        cases.append(("fine", dict(L=L, N=int(rng.integers(1, 8)), R=int(rng.integers(1, 40)), tile=S, subsweeps=K)))
+    for _ in range(3):                                                   # FINE, Poisson variant
+        S = int(rng.choice([8, 16]))
+        L = int(rng.choice([l for l in (32, 64, 128) if l >= 2 * S]))
+        cases.append(("fine", dict(L=L, N=int(rng.integers(1, 8)), R=int(rng.integers(1, 20)), tile=S, poisson=True)))
+    for _ in range(5):                                                   # LEVEL (few realizations, serial RS)
+        L = int(rng.choice([16, 32, 64]))
+        cases.append(("level", dict(L=L, N=int(rng.integers(1, 12)), R=int(rng.integers(1, 6)), tile=L)))
+    for _ in range(8):                                                   # general L: windowed pass, global pass, RSG
+        S = int(rng.choice([8, 16, 32]))
+        L = int(rng.integers(24, 260))
+        while L & (L - 1) == 0:
+            L += 1
+        K = int(rng.choice([k for k in (1, 2, 4) if S * S // k >= 32]))
+        cases.append(("simple", dict(L=L, N=int(rng.integers(1, 10)), R=int(rng.integers(1, 5)), tile=S, subsweeps=K)))
+    for _ in range(3):                                                   # MULTI
+        L = int(rng.choice([8, 16, 32]))
+        cases.append(("multi", dict(L=L, N=int(rng.integers(1, 6)), R=int(rng.integers(1, 150)), multisurface=True,
+                                    first_real=32 * int(rng.integers(0, 9)))))
+    for want, kw in cases:
+        kw = dict(kw)
+        kw.setdefault("first_real", int(rng.integers(0, 50)))
+        seed = int(rng.integers(1, 1 << 40))
+        mcs = int(rng.integers(2, 5))
+        L, N, R = kw.pop("L"), kw.pop("N"), kw.pop("R")
+        g = rsos.Rsos(L, N, R, seed, **kw)
+        o = oracle_mod.Oracle(L, N, R, seed, **kw)
+        assert g.info()["engine"] == want, (want, L, N, R, kw, g.info())
+        g.advance(mcs)
+        o.advance(mcs)
+        compare(g, o, "%s L=%d N=%d R=%d %s" % (want, L, N, R, kw))
+        g.close()
+        o.close()
