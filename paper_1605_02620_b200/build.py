@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "librsos.so")
-SOURCES = ["rsos_api.cu", "rsos_update.cu", "rsos_thread.cu", "rsos_resident.cu", "rsos_fine.cu", "rsos_multi.cu", "rsos_level.cu", "rsos_pack.cu", "rsos_reduce.cu"]
+SOURCES = ["rsos_api.cu", "rsos_update.cu", "rsos_thread.cu", "rsos_gthread.cu", "rsos_resident.cu", "rsos_fine.cu", "rsos_multi.cu", "rsos_level.cu", "rsos_pack.cu", "rsos_reduce.cu"]
 HEADERS = ["rsos_device.cuh", "rsos_internal.h", "rsos_attempt.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC,-Wall,-Wno-unknown-pragmas", "-shared"]

@@ -147,7 +147,8 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
     // engine selection (include/rsos.h)
     uint32_t engine = opt.engine;
     const bool warp_ok = !general && mode_dt && S <= 128 && N <= 31;
-    const bool thread_ok = !general && mode_dt && S <= 64 && N <= 7;
+    const bool gthread_can = general && mode_dt && gthread_ok(L, N, S, K);      // general L on the packed lattice (S = 64)
+    const bool thread_ok = (!general && mode_dt && S <= 64 && N <= 7) || gthread_can;
     const bool onchip_ok = !general && !mode_dt && L <= 128 && N <= 31;
     const uint32_t T = !mode_dt ? 0u : general ? 2u * (L / (2u * S)) : L / S;
     const uint64_t pass_tiles = mode_dt ? (uint64_t)R * (T / 2) * (T / 2) : 0;
@@ -196,8 +197,9 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
         return fail(RSOS_EUNSUP, "engine THREAD needs DT mode (2*tile <= L), tile <= 64 and N <= 7");
     if (engine == RSOS_ENGINE_ONCHIP && !onchip_ok)
         return fail(RSOS_EUNSUP, "engine ONCHIP needs RS mode (2*tile > L), L <= 128 and N <= 31");
-    if (general && engine != RSOS_ENGINE_SIMPLE)
-        return fail(RSOS_EUNSUP, "L = %u is not a power of two: only the SIMPLE engine runs the general-L schedule", L);
+    if (general && engine != RSOS_ENGINE_SIMPLE && !(engine == RSOS_ENGINE_THREAD && gthread_can))
+        return fail(RSOS_EUNSUP, "L = %u is not a power of two: the general-L schedule runs on the SIMPLE engine, and on the THREAD "
+                                 "engine when tile = 64, N <= 7 and ceil(L / T) <= 66", L);
     pl->mode_dt = mode_dt; pl->general = general; pl->T = T;
     pl->engine = engine; pl->S = S; pl->K = K; pl->pass_tiles = pass_tiles;
     pl->lanes = 0; pl->field_bits = 0;
@@ -213,7 +215,8 @@ static int make_plan(uint32_t L, uint32_t N, uint32_t R, const rsos_opts &opt, i
     }
     if (engine == RSOS_ENGINE_THREAD) {
         pl->field_bits = thread_dt_field_bits(N, S);
-        uint32_t kl = opt.lanes ? opt.lanes : thread_dt_lanes_per_tile(pass_tiles, sm_count, pl->field_bits);
+        if (general && opt.lanes > 1) return fail(RSOS_EINVAL, "opts.lanes = %u: general L runs one lane per tile", opt.lanes);
+        uint32_t kl = general ? 1u : opt.lanes ? opt.lanes : thread_dt_lanes_per_tile(pass_tiles, sm_count, pl->field_bits);
         while (!opt.lanes && 8ull * kl > (uint64_t)S * S / K) kl /= 2;                       // a batch is 8 * lanes attempts
         if (8ull * kl > (uint64_t)S * S / K)
             return fail(RSOS_EINVAL, "opts.lanes = %u needs tile^2 / subsweeps >= %u attempts per tile", kl, 8 * kl);
@@ -319,7 +322,8 @@ extern "C" int rsos_init(rsos_ctx **out, uint32_t L, uint32_t N, uint32_t R, uin
         p.FB = pl.field_bits;
         p.KL = pl.lanes;
         p.CS = pl.cluster;
-        const size_t pk_bytes = bytes / 32 * p.FB;                       // FB bits per site
+        // FB bits per site; general L: rows of ceil(L * FB / 32) words
+        const size_t pk_bytes = pl.general ? (size_t)R * L * ((L * p.FB + 31u) / 32u) * sizeof(uint32_t) : bytes / 32 * p.FB;
         INIT_TRY(cudaMalloc(&p.pk, pk_bytes), RSOS_ECUDA);
         INIT_TRY(cudaMalloc(&c->d_s1off, (size_t)R * sizeof(long long)), RSOS_ECUDA);
         INIT_TRY(cudaMalloc(&c->d_V, (size_t)R * L * sizeof(int32_t)), RSOS_ECUDA);
@@ -504,8 +508,9 @@ static int reduce_sums_packed(rsos_ctx *c)
         const unsigned long long srel2 = c->h_pk[4 * r + 1];
         const long long s1 = (long long)c->h_pk[4 * R + r] + (long long)c->h_red[4 * R + r];
         const long long num = s1 - srel;
-        const long long h00 = num >> (2 * p.lgL);
-        if ((h00 << (2 * p.lgL)) != num)
+        const long long n2 = (long long)p.L * p.L;
+        const long long h00 = p.general ? num / n2 : num >> (2 * p.lgL);
+        if (h00 * n2 != num)
             return fail(RSOS_ECUDA, "realization %zu: packed lattice is inconsistent with sum h (reconstruction not exact)", r);
         const long long lo = h00 + mn, hi = h00 + mx;
         const unsigned long long amax = (unsigned long long)((lo < 0 ? -lo : lo) > (hi < 0 ? -hi : hi) ? (lo < 0 ? -lo : lo)

@@ -31,6 +31,13 @@ cudaError_t thread_dt_configure(const Params &p);
 uint32_t thread_dt_blocks(const Params &p);
 cudaError_t thread_dt_launch(const Params &p, uint32_t u, uint32_t colour, uint32_t blocks, cudaStream_t st);
 
+// rsos_gthread.cu (lane-per-tile DT engine on the packed lattice for lattice sides that are not powers of two)
+bool gthread_ok(uint32_t L, uint32_t N, uint32_t S, uint32_t K);
+size_t gthread_smem(const Params &p);
+uint32_t gthread_blocks(const Params &p);
+cudaError_t gthread_configure(const Params &p);
+cudaError_t gthread_launch(const Params &p, uint32_t u, uint32_t colour, cudaStream_t st);
+
 // rsos_resident.cu (DT schedule with the packed lattice resident in shared memory for a whole rsos_advance)
 bool resident_ok(uint32_t L, uint32_t N, uint32_t S, uint32_t K, uint32_t csize, size_t smem_limit);
 uint32_t resident_cluster_size(uint32_t L, uint32_t N, uint32_t S, uint32_t K, uint32_t R, int sm_count, size_t smem_limit);

@@ -257,10 +257,142 @@ __global__ void anchor_kernel(const long long *s1off, const unsigned long long *
 }
 
 // =============================================================================================
+// General L (D:2b): the same packed format with a row pitch of wpr = ceil(L * FB / 32) words; site x of a row sits in
+// word x / SPW at bit (x mod SPW) * FB, the bits of the last word beyond site L - 1 are unused.  The kernels below are
+// the plain forms of the ones above (no int4 accesses, no power-of-two shifts): one thread per packed word, one warp
+// per row.  They are used only when L is not a power of two.
+// =============================================================================================
+template <int FB>
+__global__ void __launch_bounds__(256) gpack_kernel(const int32_t *__restrict__ h, uint32_t *__restrict__ pk, uint32_t L,
+                                                    uint32_t wpr, size_t nwords)
+{
+    constexpr uint32_t SPW = 32 / FB, M = (1u << FB) - 1u;
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nwords) return;
+    const size_t row = i / wpr;
+    const uint32_t w = (uint32_t)(i - row * wpr);
+    const int32_t *src = h + row * L;
+    uint32_t out = 0;
+#pragma unroll
+    for (uint32_t k = 0; k < SPW; ++k) {
+        const uint32_t x = w * SPW + k;
+        if (x < L) out |= ((uint32_t)src[x] & M) << (k * FB);
+    }
+    pk[i] = out;
+}
+
+template <int FB, bool WRITE>
+__global__ void __launch_bounds__(256) gunpack_rows_kernel(const uint32_t *__restrict__ pk, const int32_t *__restrict__ V,
+                                                           const int32_t *__restrict__ h00, int32_t *__restrict__ h,
+                                                           unsigned long long *__restrict__ srel, uint32_t L, uint32_t wpr,
+                                                           uint32_t nrows)
+{
+    constexpr uint32_t SPW = 32 / FB, M = (1u << FB) - 1u;
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const uint32_t row = blockIdx.x * 8u + warp;
+    const bool row_ok = row < nrows;                               // warp-uniform
+    const uint32_t wpt = (wpr + 31u) / 32u;
+    const uint32_t w0 = lane * wpt;
+    const uint32_t nw = (row_ok && w0 < wpr) ? min(wpt, wpr - w0) : 0u;
+    const uint32_t *rowp = pk + (size_t)(row_ok ? row : 0u) * wpr;
+    const uint32_t rl = (row_ok ? row : 0u) / L;
+
+    uint32_t prevf = 0;                                            // the field before my first site (site 0: itself)
+    if (nw) prevf = (w0 == 0u) ? (rowp[0] & M) : (rowp[w0 - 1u] >> (32 - FB));
+    int32_t tot = 0;
+    {
+        uint32_t pf = prevf;
+        for (uint32_t i = 0; i < nw; ++i) {
+            const uint32_t w = rowp[w0 + i];
+#pragma unroll
+            for (uint32_t k = 0; k < SPW; ++k) {
+                if ((w0 + i) * SPW + k < L) {
+                    const uint32_t f = (w >> (k * FB)) & M;
+                    tot += sdiff<FB>(f, pf);
+                    pf = f;
+                }
+            }
+        }
+    }
+    int32_t incl = tot;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int32_t n = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+        if ((int)lane >= o) incl += n;
+    }
+    int32_t run = incl - tot;
+    if (row_ok) run += V[row];
+    if (WRITE && row_ok) run += h00[rl];
+    long long acc = 0;
+    unsigned long long acc2 = 0;
+    int32_t mn = 0x7FFFFFFF, mx = -0x7FFFFFFF - 1;
+    {
+        uint32_t pf = prevf;
+        for (uint32_t i = 0; i < nw; ++i) {
+            const uint32_t w = rowp[w0 + i];
+#pragma unroll
+            for (uint32_t k = 0; k < SPW; ++k) {
+                const uint32_t x = (w0 + i) * SPW + k;
+                if (x < L) {
+                    const uint32_t f = (w >> (k * FB)) & M;
+                    run += sdiff<FB>(f, pf);
+                    pf = f;
+                    if (WRITE) h[(size_t)row * L + x] = run;
+                    else {
+                        acc += run;
+                        acc2 += (unsigned long long)((long long)run * run);
+                        mn = min(mn, run);
+                        mx = max(mx, run);
+                    }
+                }
+            }
+        }
+    }
+    if (!WRITE) {
+#pragma unroll
+        for (int o = 16; o; o >>= 1) {
+            acc += __shfl_xor_sync(0xFFFFFFFFu, acc, o);
+            acc2 += __shfl_xor_sync(0xFFFFFFFFu, acc2, o);
+            mn = min(mn, __shfl_xor_sync(0xFFFFFFFFu, mn, o));
+            mx = max(mx, __shfl_xor_sync(0xFFFFFFFFu, mx, o));
+        }
+        if (lane == 0 && row_ok) {                                  // a block's 8 rows may belong to two realizations: per warp
+            unsigned long long *d = srel + 4 * (size_t)rl;
+            if (acc != 0) atomicAdd(d, (unsigned long long)acc);
+            if (acc2 != 0) atomicAdd(d + 1, acc2);
+            if (mn <= mx) {
+                atomicMin(reinterpret_cast<long long *>(d + 2), (long long)mn);
+                atomicMax(reinterpret_cast<long long *>(d + 3), (long long)mx);
+            }
+        }
+    }
+}
+
+// h00[r] = (s1off[r] + accepted[r] - srel[4r]) / L^2 for any L; must divide exactly and fit int32.
+__global__ void ganchor_kernel(const long long *s1off, const unsigned long long *accepted, const unsigned long long *srel,
+                               int32_t *h00, long long n2, uint32_t R, uint32_t *err)
+{
+    const uint32_t r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= R) return;
+    const long long num = s1off[r] + (long long)accepted[r] - (long long)srel[4 * (size_t)r];
+    const long long q = num / n2;
+    if (q * n2 != num || q > 0x7FFFFFFFll || q < -0x80000000ll) atomicOr(err, ERR_RECONSTRUCT);
+    h00[r] = (int32_t)q;
+}
+
+// =============================================================================================
 // Host-side launchers
 // =============================================================================================
 cudaError_t launch_pack(const Params &p, cudaStream_t st)
 {
+    if (p.general) {
+        const uint32_t wpr = (p.L * p.FB + 31u) / 32u;
+        const size_t nw = (size_t)p.R * p.L * wpr;
+        const uint32_t gb = (uint32_t)((nw + 255) / 256);
+        if (p.FB == 2) gpack_kernel<2><<<gb, 256, 0, st>>>(p.h, p.pk, p.L, wpr, nw);
+        else gpack_kernel<4><<<gb, 256, 0, st>>>(p.h, p.pk, p.L, wpr, nw);
+        return cudaGetLastError();
+    }
     const size_t nwords = (size_t)p.R * p.L * p.L * p.FB / 32;
     const uint32_t blocks = (uint32_t)((nwords + 255) / 256);
     if (p.FB == 2) pack_kernel<2><<<blocks, 256, 0, st>>>(p.h, p.pk, nwords);
@@ -279,6 +411,18 @@ cudaError_t launch_s1off(const Params &p, const unsigned long long *d_red, long 
 // materialising the int32 heights.  Scratch: d_V (R*L int32).  3 kernels.
 cudaError_t launch_packed_sums(const Params &p, int32_t *d_V, unsigned long long *d_srel, cudaStream_t st)
 {
+    if (p.general) {
+        const uint32_t gwpr = (p.L * p.FB + 31u) / 32u, gnrows = p.R * p.L;
+        srel_init_kernel<<<(p.R + 127) / 128, 128, 0, st>>>(d_srel, p.R);
+        if (p.FB == 2) {
+            unpack_col_kernel<2><<<p.R, 256, 0, st>>>(p.pk, d_V, p.L, gwpr);
+            gunpack_rows_kernel<2, false><<<(gnrows + 7u) / 8u, 256, 0, st>>>(p.pk, d_V, nullptr, p.h, d_srel, p.L, gwpr, gnrows);
+        } else {
+            unpack_col_kernel<4><<<p.R, 256, 0, st>>>(p.pk, d_V, p.L, gwpr);
+            gunpack_rows_kernel<4, false><<<(gnrows + 7u) / 8u, 256, 0, st>>>(p.pk, d_V, nullptr, p.h, d_srel, p.L, gwpr, gnrows);
+        }
+        return cudaGetLastError();
+    }
     const uint32_t wpr = p.L * p.FB / 32;
     const uint32_t nrows = p.R * p.L;
     const uint32_t rblocks = wpr >= 256u ? nrows : (nrows + 7u) / 8u;
@@ -303,6 +447,14 @@ cudaError_t launch_unpack(const Params &p, const long long *d_s1off, int32_t *d_
     const uint32_t rblocks = wpr >= 256u ? nrows : (nrows + 7u) / 8u;
     cudaError_t e = launch_packed_sums(p, d_V, d_srel, st);
     if (e != cudaSuccess) return e;
+    if (p.general) {
+        const uint32_t gwpr = (p.L * p.FB + 31u) / 32u;
+        ganchor_kernel<<<(p.R + 127) / 128, 128, 0, st>>>(d_s1off, p.accepted, d_srel, d_h00, (long long)p.L * p.L, p.R, p.err);
+        if (p.FB == 2) gunpack_rows_kernel<2, true><<<(nrows + 7u) / 8u, 256, 0, st>>>(p.pk, d_V, d_h00, p.h, d_srel, p.L, gwpr, nrows);
+        else gunpack_rows_kernel<4, true><<<(nrows + 7u) / 8u, 256, 0, st>>>(p.pk, d_V, d_h00, p.h, d_srel, p.L, gwpr, nrows);
+        *launches = 5;
+        return cudaGetLastError();
+    }
     anchor_kernel<<<(p.R + 127) / 128, 128, 0, st>>>(d_s1off, p.accepted, d_srel, d_h00, 2 * p.lgL, p.R, p.err);
     if (p.FB == 2) unpack_rows_kernel<2, true><<<rblocks, 256, 0, st>>>(p.pk, d_V, d_h00, p.h, d_srel, p.L, wpr, nrows);
     else unpack_rows_kernel<4, true><<<rblocks, 256, 0, st>>>(p.pk, d_V, d_h00, p.h, d_srel, p.L, wpr, nrows);

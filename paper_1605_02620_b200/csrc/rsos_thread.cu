@@ -326,15 +326,20 @@ uint32_t thread_dt_lanes_per_tile(uint64_t pass_tiles, int sm_count, uint32_t fi
 
 size_t thread_dt_smem(const Params &p)
 {
+    if (p.general) return gthread_smem(p);
     size_t sm = 0;
     thread_dispatch(p, 0, 0, 0, nullptr, 0, &sm);
     return sm;
 }
 
-cudaError_t thread_dt_configure(const Params &p) { return thread_dispatch(p, 0, 0, 0, nullptr, 1, nullptr); }
+cudaError_t thread_dt_configure(const Params &p)
+{
+    return p.general ? gthread_configure(p) : thread_dispatch(p, 0, 0, 0, nullptr, 1, nullptr);
+}
 
 uint32_t thread_dt_blocks(const Params &p)
 {
+    if (p.general) return gthread_blocks(p);
     const uint32_t T = p.L >> p.lgS, half = T >> 1;
     const uint64_t tiles = (uint64_t)p.R * half * half;
     const uint32_t nt = 32u / p.KL;
@@ -343,6 +348,7 @@ uint32_t thread_dt_blocks(const Params &p)
 
 cudaError_t thread_dt_launch(const Params &p, uint32_t u, uint32_t colour, uint32_t blocks, cudaStream_t st)
 {
+    if (p.general) return gthread_launch(p, u, colour, st);     // lattice side not a power of two: rsos_gthread.cu
     return thread_dispatch(p, u, colour, blocks, st, 2, nullptr);
 }
 

@@ -122,8 +122,9 @@ def test_plan_picks_engines_lanes_and_site_width(lib_path):
         m.plan(1024, 1, 128, subsweeps=128, engine=m.ENGINE_THREAD, lanes=8)         # a batch of 64 attempts does not fit
     assert e.value.code == -1
     # lattice sides that are not powers of two: the general-L schedule, SIMPLE engine
-    p = m.plan(9605, 1, 128)
-    assert (p["mode"], p["engine"], p["S"], p["pass_tiles"]) == ("DT", "simple", 64, 128 * 75 * 75)
+    p = m.plan(9605, 1, 128)                      # tiles of 64 / 65 sites fit the packed windows: lane-per-tile engine
+    assert (p["mode"], p["engine"], p["S"], p["pass_tiles"], p["lanes"], p["packed_bits"]) == ("DT", "thread", 64, 128 * 75 * 75, 1, 2)
+    assert m.plan(9605, 9, 1)["engine"] == "simple" and m.plan(150, 1, 4)["engine"] == "simple"   # N > 7; 75-site tiles
     p = m.plan(100, 1, 4)
     assert (p["mode"], p["engine"], p["S"]) == ("RS", "simple", 100)
     # fewer SMs: the same pass reaches six warps per SM with fewer lanes
