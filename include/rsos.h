@@ -127,13 +127,16 @@ typedef struct rsos_opts {
  *   L     lattice side, 4 <= L <= 65536 (periodic in both directions, reading Q2).  Powers of two run the
  *         schedule D:2 on every engine; any other L (the paper's L = 9605) runs the general-L schedule
  *         D:2b -- tiles of two sizes that divide the lattice, sites drawn by an exactly uniform bounded
- *         draw -- on the SIMPLE engine only (int32 heights; byte tile windows in shared memory when N <= 7)
+ *         draw -- on the THREAD engine (packed lattice, one lane per tile) when tile = 64, N <= 7 and
+ *         ceil(L / T) <= 66 with T = 2 floor(L / 128) (every L >= 4224, e.g. 9605), else on the SIMPLE engine
+ *         (int32 heights; byte tile windows in shared memory when N <= 7)
  *   N     height-difference bound of Eq. (6), 1 <= N <= 127
  *   R     number of independent realizations, >= 1, R*L*L*4 bytes must fit on the device
  *   seed  Philox key (low word, high word)
  *   opts  host, may be NULL
  * Errors: RSOS_EINVAL (L, N, R, tile, subsweeps, engine, misaligned d_heights), RSOS_EUNSUP
- * (engine cannot run the mode, or an engine other than AUTO / SIMPLE with L not a power of two),
+ * (engine cannot run the mode; L not a power of two: engines other than AUTO, SIMPLE and -- under the
+ * condition above -- THREAD),
  * RSOS_ENOMEM, RSOS_ECUDA.
  */
 int rsos_init(rsos_ctx **ctx, uint32_t L, uint32_t N, uint32_t R, uint64_t seed, const rsos_opts *opts);
