@@ -8,7 +8,8 @@ batch: `mcs_per_step` Monte-Carlo steps of rsos_advance (Philox draws, origin dr
 attempt loop, write-back) followed by one rsos_width (int64 width reduction, result read to host).
 The headline workload is BASELINE.json configs[1] (C2: L=1024, N=1, 128 realizations, DT(64,1)).  The
 same run then times, with the same fields under "extra", the other north_star config (C4: L=2^15, one
-surface) and short legs on C3 (N=1, 2), C5 (L=64..512) and C1, so that every BASELINE config has a
+surface), short legs on C3 (N=1, 2), C5 (L=64..512) and C1, and one on the paper's own largest lattice
+(X1: L=9605, not a power of two), so that every BASELINE config has a
 number the driver's own run produced.  Nothing is flushed between steps: a step sweeps the same
 resident lattice 4K * mcs_per_step times exactly as a production run does; `config.l2` says what is
 resident where.
@@ -68,7 +69,7 @@ def parse():
 
 
 # legs of the default run besides the headline workload: the other north_star config (C4) and short legs on the rest
-EXTRA_LEGS = ("C4", "C2", "C3", "C3/N=2", "C5", "C5/L=128", "C5/L=256", "C5/L=512", "C1")
+EXTRA_LEGS = ("C4", "C2", "C3", "C3/N=2", "C5", "C5/L=128", "C5/L=256", "C5/L=512", "C1", "X1")
 
 
 def workload(args):
@@ -279,7 +280,7 @@ def leg_config(name):
             c["R"] = workloads.c5_realizations(c["L"])
             c["mcs"] = workloads.c5_mcs(c["L"])
     # MCS per step: 10-40 ms of device work per step, far above launch and event overheads
-    dflt = {"C1": 1000, "C2": 32, "C3": 16, "C4": 4, "C5": 256}[base]
+    dflt = {"C1": 1000, "C2": 32, "C3": 16, "C4": 4, "C5": 256, "X1": 8}[base]
     if base == "C5" and c["L"] > 64:
         dflt = {128: 256, 256: 256, 512: 128}[c["L"]]
     c["mcs_per_step"] = dflt

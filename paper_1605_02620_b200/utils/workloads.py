@@ -13,6 +13,9 @@ CONFIGS = {
     "C3": dict(L=2048, N=1, R=64, mcs=5_000, seed=1, tile=64, subsweeps=1),        # N in 1..4
     "C4": dict(L=32768, N=1, R=1, mcs=2_000, seed=1, tile=64, subsweeps=1),
     "C5": dict(L=64, N=1, R=4096, mcs=15_521, seed=1, tile=64, subsweeps=4),       # L in 64..512, N in 1,2
+    # not a BASELINE config: the paper's own largest system (L = 9605, t = 1e5 MCS, 128 realizations),
+    # a lattice side that is not a power of two (general-L schedule), at 4 realizations
+    "X1": dict(L=9605, N=1, R=4, mcs=100_000, seed=1, tile=64, subsweeps=1),
 }
 
 
