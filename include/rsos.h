@@ -166,6 +166,52 @@ int rsos_sums(rsos_ctx *ctx, int64_t *S1, uint64_t *S2, int64_t *accepted);
 int rsos_width(rsos_ctx *ctx, double *W2, double *hmean);
 
 /*
+ * rsos_sums_static -- the sums of rsos_sums (Eq. 2) for code that is not allowed to allocate.
+ *
+ * Who this is for.  rsos_init obtains its reduction buffers with cudaMalloc, and some users of the width sums cannot
+ * make that call, or any call that ends in it: an analysis step that runs inside a job whose device memory has been
+ * handed over in full to another pool (a framework's caching allocator sized to the whole GPU leaves a raw cudaMalloc
+ * nothing to take, so it fails), and a measurement loop that may not stall, because cudaMalloc and cudaFree wait for
+ * the whole device and so serialise every stream of the process.  Such callers already own their buffers; this call
+ * works entirely inside them plus one fixed array that belongs to the library.
+ *
+ * What it does.  d_heights holds R surfaces of L x L int32 heights on the CURRENT device (h[r][y][x], row-major; the
+ * layout of rsos_device_heights, whose pointer may be passed straight in).  The call enqueues on `stream` the same
+ * reduction kernel rsos_sums uses and writes, for r < R:
+ *     d_S1[r]     = sum_x h(x)        (int64)
+ *     d_S2[r]     = sum_x h(x)^2      (uint64, exact modulo 2^64)
+ *     d_maxabs[r] = max_x |h(x)|      (uint32)
+ * S2 is the true sum whenever maxabs^2 * L^2 < 2^64 (the condition rsos_sums turns into RSOS_ERANGE; here the caller
+ * checks it, because reading the value back would force a synchronisation).  No context is needed, nothing is read
+ * back to the host, and the call returns without waiting for the GPU.
+ *
+ *   d_heights  DEVICE, in: R*L*L int32, 16-byte aligned (4-byte if L*L is not a multiple of 4), not modified
+ *   L          4 <= L <= 65536, any value
+ *   R          1 <= R <= RSOS_STATIC_MAX_R; more is refused with RSOS_EINVAL and a message naming the limit
+ *   d_S1, d_S2, d_maxabs   DEVICE, out: R elements each, caller-owned, any may be NULL (not all three)
+ *   stream     cudaStream_t to enqueue on; NULL = the legacy default stream
+ *
+ * The fixed array.  The kernel accumulates with atomics into 32 bytes per realization.  For this call those bytes sit
+ * in a file-scope __device__ array of RSOS_STATIC_MAX_R rows (128 KiB) compiled into librsos: every GPU on which the
+ * library's code is loaded carries that array until the process exits, whether or not this function is ever called.
+ * The call itself uses no cudaMalloc, cudaFree, cudaMallocHost or any routine that allocates.
+ *   - First call on each device: the function looks up where that device keeps the array (cudaGetSymbolAddress, which
+ *     may also make the runtime load the library's device code there) and remembers the answer; later calls on that
+ *     device skip this.  Make this first call during start-up, with the intended device current, and before any
+ *     stream capture is begun on that device.
+ *   - The array is shared by all calls and keeps whatever the previous call left in it.  Each call therefore zeroes, on
+ *     `stream`, exactly the rows it is about to use before the kernel adds into them; nothing else needs clearing.
+ *   - Because of that sharing, two calls whose GPU work can overlap -- different streams, or two host threads -- add
+ *     into the same rows and both get wrong sums.  Keep all calls for one device on one stream, or order them with
+ *     events.  Calls on different devices do not interact.
+ *
+ * Errors: RSOS_EINVAL (NULL or misaligned pointer, L or R out of range -- nothing is enqueued), RSOS_ECUDA.
+ */
+#define RSOS_STATIC_MAX_R 4096u
+int rsos_sums_static(const int32_t *d_heights, uint32_t L, uint32_t R, int64_t *d_S1, uint64_t *d_S2,
+                     uint32_t *d_maxabs, void *stream);
+
+/*
  * rsos_moments -- (Eq. 13-15) exact central power sums about the
  * integer base b[r] = floor(S1[r] / L^2):  M[r][k-1] = sum_x (h(x) - b[r])^k for k = 1..4 as
  * signed 128-bit integers stored little-endian in two uint64 words (lo, hi): out[r][k-1][2].

@@ -19,7 +19,8 @@ RSOS_OK, RSOS_EINVAL, RSOS_ERANGE, RSOS_ENOMEM, RSOS_ECUDA, RSOS_EUNSUP = 0, -1,
 # every symbol include/rsos.h declares (tests check the .so exports exactly these)
 SYMBOLS = ("rsos_init", "rsos_advance", "rsos_sums", "rsos_width", "rsos_moments", "rsos_height_moments", "rsos_get_heights",
            "rsos_set_state", "rsos_time", "rsos_info", "rsos_device_heights", "rsos_kernel_time",
-           "rsos_free", "rsos_last_error", "rsos_philox", "rsos_plan")
+           "rsos_free", "rsos_last_error", "rsos_philox", "rsos_plan", "rsos_sums_static")
+STATIC_MAX_R = 4096                # RSOS_STATIC_MAX_R of include/rsos.h
 
 
 class RsosOpts(C.Structure):
@@ -59,6 +60,7 @@ def load():
     l.rsos_device_heights.argtypes = [vp, C.POINTER(vp)]
     l.rsos_kernel_time.argtypes = [vp, ci, C.POINTER(C.c_double), C.POINTER(u64)]
     l.rsos_philox.argtypes = [vp, vp, vp, u32]
+    l.rsos_sums_static.argtypes = [vp, u32, u32, vp, vp, vp, vp]
     for name in SYMBOLS:
         getattr(l, name).restype = ci
     l.rsos_free.restype = None
@@ -89,6 +91,18 @@ def philox(ctr, key):
     out = np.empty_like(ctr)
     _check(load().rsos_philox(ctr.ctypes.data, key.ctypes.data, out.ctypes.data, len(ctr)))
     return out
+
+
+def sums_static(d_heights, L, R, d_S1=None, d_S2=None, d_maxabs=None, stream=None):
+    """rsos_sums_static: S1, S2 and max |h| of R surfaces that already sit in device memory, written to device arrays
+    the caller owns, without any allocation by the library (see include/rsos.h: it exists for callers that cannot
+    reach the CUDA allocator -- all device memory belongs to another pool -- or cannot afford its device-wide stall).
+
+    Every pointer is a device address as a Python int (tensor.data_ptr()); the outputs hold R int64 / uint64 / uint32.
+    R <= STATIC_MAX_R.  Asynchronous on `stream` (a cudaStream_t as int, None = the legacy default stream); all calls
+    on a device share one fixed scratch array, so calls that could overlap on the GPU must be ordered by the caller.
+    The first call on a device does a one-time address look-up; make it before any stream capture."""
+    _check(load().rsos_sums_static(d_heights or None, int(L), int(R), d_S1 or None, d_S2 or None, d_maxabs or None, stream or None))
 
 
 class Rsos:

@@ -568,6 +568,27 @@ extern "C" int rsos_sums(rsos_ctx *c, int64_t *S1, uint64_t *S2, int64_t *accept
     return RSOS_OK;
 }
 
+// Context-free and allocation-free: see include/rsos.h.  Argument checks here, the work in rsos_reduce.cu.
+extern "C" int rsos_sums_static(const int32_t *d_heights, uint32_t L, uint32_t R, int64_t *d_S1, uint64_t *d_S2,
+                                uint32_t *d_maxabs, void *stream)
+{
+    if (!d_heights) return fail(RSOS_EINVAL, "d_heights is NULL");
+    if (L < 4 || L > 65536) return fail(RSOS_EINVAL, "L = %u must be in [4, 65536]", L);
+    if (R < 1) return fail(RSOS_EINVAL, "R must be >= 1");
+    if (R > RSOS_STATIC_MAX_R)
+        return fail(RSOS_EINVAL, "R = %u exceeds RSOS_STATIC_MAX_R = %u, the number of realizations the library's fixed scratch "
+                                 "array holds: split the surfaces over several calls, or use rsos_sums on a context", R,
+                    RSOS_STATIC_MAX_R);
+    if (!d_S1 && !d_S2 && !d_maxabs) return fail(RSOS_EINVAL, "d_S1, d_S2 and d_maxabs are all NULL: nothing to write");
+    const bool vec = ((uint64_t)L * L) % 4 == 0;
+    if ((uintptr_t)d_heights & (vec ? 15u : 3u)) return fail(RSOS_EINVAL, "d_heights must be %u-byte aligned", vec ? 16u : 4u);
+    if (((uintptr_t)d_S1 & 7u) || ((uintptr_t)d_S2 & 7u) || ((uintptr_t)d_maxabs & 3u))
+        return fail(RSOS_EINVAL, "d_S1 / d_S2 must be 8-byte aligned and d_maxabs 4-byte aligned");
+    CUDA_TRY(launch_sums_static(d_heights, L, R, reinterpret_cast<long long *>(d_S1), reinterpret_cast<unsigned long long *>(d_S2),
+                                d_maxabs, static_cast<cudaStream_t>(stream)));
+    return RSOS_OK;
+}
+
 extern "C" int rsos_width(rsos_ctx *c, double *W2, double *hmean)
 {
     if (!c) return fail(RSOS_EINVAL, "ctx is NULL");

@@ -83,5 +83,9 @@ cudaError_t launch_violations(const int32_t *h, uint32_t L, uint32_t lgL, uint32
 // out: per realization 8 x uint64: M1..M4 as (lo, hi) two's-complement 128-bit
 cudaError_t launch_moments(const int32_t *h, uint32_t L, uint32_t R, const long long *d_base,
                            unsigned long long *d_out, int sm_count, cudaStream_t st);
+// rsos_sums_static: launch_sums into the library's fixed device array (no allocation), results copied to the three
+// caller-owned device arrays (any of them may be null); R <= RSOS_STATIC_MAX_R, current device, enqueued on st
+cudaError_t launch_sums_static(const int32_t *h, uint32_t L, uint32_t R, long long *d_S1, unsigned long long *d_S2,
+                               unsigned int *d_maxabs, cudaStream_t st);
 
 }  // namespace rsos

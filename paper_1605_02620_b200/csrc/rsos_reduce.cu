@@ -4,6 +4,9 @@
 // exact integers S1 = sum h (int64) and S2 = sum h^2 (uint64); the division happens once on the
 // host from a 128-bit numerator (rsos_api.cu).  Integer adds commute, so the block order and the
 // atomics do not affect the result.  HBM-bound: 4 B per site, int4 loads, grid = multiple of SMs.
+#include <mutex>
+
+#include "../../include/rsos.h"
 #include "rsos_internal.h"
 
 namespace rsos {
@@ -192,6 +195,83 @@ cudaError_t launch_violations(const int32_t *h, uint32_t L, uint32_t lgL, uint32
         const uint32_t cnt = nr - r0 < 65535 ? nr - r0 : 65535;
         violations_kernel<<<dim3(bx ? bx : 1, cnt), RED_THREADS, 0, st>>>(h + (size_t)r0 * n, L, lgL, (int32_t)N, d_bad);
     }
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------
+// rsos_sums_static (include/rsos.h): the width sums for callers that must stay away from the CUDA
+// allocator.  Same reduction as above (sums_kernel, Eq. 2), but the per-realization
+// accumulators it adds into live in a fixed array that is part of the loaded library image
+// instead of in a buffer some rsos_init obtained with cudaMalloc.
+//
+// g_static_red is a DEVICE object.  In host code its name only identifies the symbol; it is not an
+// address a kernel can use.  static_scratch() asks the runtime for the real address once per
+// device (cudaGetSymbolAddress, with that device current) and everything below works with that
+// pointer.  One array per device, shared by every call and never cleared behind the caller's back:
+// launch_sums zeroes the R rows it is going to use on the caller's stream before the kernel adds
+// into them, and two calls whose work overlaps on the GPU (different streams, or two host threads)
+// would add into the same rows -- the header says so.
+// ---------------------------------------------------------------------------------------------
+constexpr uint32_t STATIC_MAX_R = RSOS_STATIC_MAX_R;
+constexpr int STATIC_MAX_DEVICES = 64;
+
+static __device__ __align__(256) unsigned long long g_static_red[(size_t)STATIC_MAX_R * 4];   // 32 B per realization: 128 KiB
+
+struct StaticScratch {
+    bool ready = false;
+    unsigned long long *ptr = nullptr;
+    int sm_count = 0;
+};
+static StaticScratch g_static[STATIC_MAX_DEVICES];
+static std::mutex g_static_mutex;
+
+// The current device's copy of g_static_red and its SM count (looked up on the first call per device).
+static cudaError_t static_scratch(unsigned long long **ptr, int *sm_count)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticScratch &s = g_static[dev];
+    if (!s.ready) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_static_red);
+        if (e != cudaSuccess) return e;
+        int sms = 0;
+        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return e;
+        s.ptr = static_cast<unsigned long long *>(p);
+        s.sm_count = sms;
+        s.ready = true;
+    }
+    *ptr = s.ptr;
+    *sm_count = s.sm_count;
+    return cudaSuccess;
+}
+
+// Accumulator rows (S1, S2, max |h|, unused) -> the caller's three output arrays.
+__global__ void __launch_bounds__(RED_THREADS) static_finish_kernel(const unsigned long long *__restrict__ red, uint32_t R,
+                                                                    long long *S1, unsigned long long *S2, unsigned int *maxabs)
+{
+    const uint32_t r = blockIdx.x * RED_THREADS + threadIdx.x;
+    if (r >= R) return;
+    if (S1) S1[r] = (long long)red[4 * (size_t)r];
+    if (S2) S2[r] = red[4 * (size_t)r + 1];
+    if (maxabs) maxabs[r] = (unsigned int)red[4 * (size_t)r + 2];
+}
+
+cudaError_t launch_sums_static(const int32_t *h, uint32_t L, uint32_t R, long long *d_S1, unsigned long long *d_S2,
+                               unsigned int *d_maxabs, cudaStream_t st)
+{
+    if (R < 1 || R > STATIC_MAX_R) return cudaErrorInvalidValue;          // rsos_sums_static reports this with a message first
+    unsigned long long *red = nullptr;
+    int sm_count = 0;
+    cudaError_t e = static_scratch(&red, &sm_count);
+    if (e != cudaSuccess) return e;
+    e = launch_sums(h, L, R, red, sm_count, st);                          // clears rows 0..R-1 of red on st, then sums_kernel
+    if (e != cudaSuccess) return e;
+    static_finish_kernel<<<(R + RED_THREADS - 1) / RED_THREADS, RED_THREADS, 0, st>>>(red, R, d_S1, d_S2, d_maxabs);
     return cudaGetLastError();
 }
 
