@@ -6,13 +6,18 @@
 A *step* is one pass of the whole hot path over one
 batch: `mcs_per_step` Monte-Carlo steps of rsos_advance (Philox draws, origin draw, tile staging,
 attempt loop, write-back) followed by one rsos_width (int64 width reduction, result read to host).
-The headline workload is BASELINE.json configs[1] (C2: L=1024, N=1, 128 realizations, DT(64,1)).  The
-same run then times, with the same fields under "extra", the other north_star config (C4: L=2^15, one
-surface), short legs on C3 (N=1, 2), C5 (L=64..512) and C1, and one on the paper's own largest lattice
-(X1: L=9605, not a power of two), so that every BASELINE config has a
-number the driver's own run produced.  Nothing is flushed between steps: a step sweeps the same
-resident lattice 4K * mcs_per_step times exactly as a production run does; `config.l2` says what is
-resident where.
+The headline workload is BASELINE.json configs[1] (C2: L=1024, N=1, 128 realizations, DT(64,1)), seed 1.
+
+Output.  The LAST stdout line is ONE compact JSON object (< 2 KB, checked before printing: the driver keeps only a few
+KB of output) that carries the C2 headline alone, plus two small side numbers: "c4" (the other north_star config,
+L=2^15, one surface) and "c2_seeds4" (configs[1] as BASELINE.json words it, "seeds 1..4": four contexts on four
+streams, so a colour pass has 32768 tiles in flight instead of 8192).  Everything else -- the full record of every leg
+with engine info, clocks and per-kernel numbers, and with --all-legs the legs on C3, C5 and C1 -- is written to the
+side file bench_legs.json (git-ignored) and never printed.  Nothing is flushed between steps: a step sweeps the same
+resident lattice 4K * mcs_per_step times exactly as a production run does; `config.l2` says so.
+
+`value` is the MEDIAN of --reps (default 3) timed regions of exactly --steps steps each (median of at least
+three timed runs); `ms_per_step` belongs to that median region.
 
 value     whole-job attempts/s with the lattice resident on the device (device-timed with CUDA events
           on the stream the kernels run on, barrier + synchronize on both sides, max over ranks).
@@ -24,9 +29,11 @@ roofline  dominant kernel (the update kernel), bound "alu": attempts/s of the up
           (DESIGN.md section 6).  `int32_equiv_sweep` keeps north_star's other candidate -- 8.25 B per
           attempt as if the lattice were int32 -- as a labelled equivalent rate; `traffic` is the DRAM
           bytes per launch ncu measured.
-cpu_baseline / --impl reference: the CPU oracle as it stands, on a bounded sample of the workload.
+cpu_baseline / --impl reference: the CPU oracle as it stands, on a bounded sample of the workload; cpu_baseline also
+          carries the two other oracle timings SURVEY 8(d) lists: C1 in full on one thread and a cut-down C4
+          (L=32768, 2 MCS) on all cores.
 N > 1: replicas only: rank i runs realizations [i*R, (i+1)*R), no collective
-on the data path; scaling is weak; the extra legs are skipped.
+on the data path; scaling is weak; the side legs are skipped.
 """
 import argparse
 import json
@@ -62,14 +69,19 @@ def parse():
     ap.add_argument("--subsweeps", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--no-extra", action="store_true", help="skip the legs on the other BASELINE configs")
-    ap.add_argument("--extra-steps", type=int, default=5, help="timed steps of each extra leg")
+    ap.add_argument("--no-extra", action="store_true", help="skip the side legs (C4, C2 with seeds 1..4)")
+    ap.add_argument("--all-legs", action="store_true", help="also time C3, C3/N=2, C5 (L=64..512), C1 and X1 (side file only)")
+    ap.add_argument("--extra-steps", type=int, default=5, help="timed steps of each side leg")
+    ap.add_argument("--reps", type=int, default=3, help="timed regions of --steps steps each; the median is reported")
+    ap.add_argument("--legs-file", default=os.path.join(ROOT, "bench_legs.json"), help="where the full per-leg records go")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
 
 
-# legs of the default run besides the headline workload: the other north_star config (C4) and short legs on the rest
+# side legs: the default run times the other north_star config (C4); --all-legs adds the rest (side file only)
+DEFAULT_LEGS = ("C4",)
 EXTRA_LEGS = ("C4", "C2", "C3", "C3/N=2", "C5", "C5/L=128", "C5/L=256", "C5/L=512", "C1", "X1")
+MAX_LINE_BYTES = 2048         # the driver keeps a few KB of output: the final line must fit whole
 
 
 def workload(args):
@@ -95,20 +107,18 @@ def cpu_model():
 
 
 def l2_note(c, info):
-    """Timing rule: say whether the inputs exceed L2 or are flushed.  A step sweeps the same resident lattice
-    mcs_per_step * 4K times, exactly as a production run does, so nothing is flushed; what is resident is stated."""
+    """Engine-dependent residency note (full leg record only; `config` must be the same string for both arms)."""
     int32_mib = c["R"] * c["L"] ** 2 * 4 / 2 ** 20
-    if info and info.get("engine") == "resident":
-        return ("lattice resident in shared memory for all %d MCS of a step (packed copy in HBM %.0f MiB, touched once per "
-                "rsos_advance); nothing to flush" % (c["mcs_per_step"], int32_mib * info.get("packed_bits", 2) / 32))
-    if info and info.get("engine") == "thread":
-        fb = 2 if (c["N"] <= 1 and c["tile"] >= 16) else 4
-        work = int32_mib * fb / 32
-        return ("working lattice %.0f MiB per GPU (%d bits/site, DESIGN.md section 5; int32 view %.0f MiB) vs 126 MB L2: %s; "
-                "no flush: consecutive sweeps of a production run see the same residency" % (
-                    work, fb, int32_mib, "larger than L2" if work * 2 ** 20 > 126e6 else "L2-resident by design"))
-    return "state %.0f MiB int32 per GPU vs 126 MB L2: %s" % (
-        int32_mib, "inputs larger than L2, no flush" if int32_mib * 2 ** 20 > 2 * 126e6 else "L2/on-chip resident by design")
+    if info and info.get("engine") in ("resident", "fine", "onchip", "level", "multi"):
+        return "lattice in shared memory for all %d MCS of a step; int32 view %.0f MiB" % (c["mcs_per_step"], int32_mib)
+    if info and info.get("packed_bits"):
+        work = int32_mib * info["packed_bits"] / 32
+        return "working lattice %.0f MiB (%d bits/site; int32 view %.0f MiB) vs 126 MB L2: %s" % (
+            work, info["packed_bits"], int32_mib, "larger than L2" if work * 2 ** 20 > 126e6 else "L2-resident")
+    return "state %.0f MiB int32 vs 126 MB L2" % int32_mib
+
+
+L2_RULE = "no flush: sweeps revisit the resident lattice as in production (DESIGN.md 6)"
 
 
 def traffic_note(workload_name, info):
@@ -133,12 +143,12 @@ def config_dict(args, c, n_gpus, info=None):
 
 def config_dict_for(name, c, n_gpus, info=None):
     mode = "RS" if 2 * c["tile"] > c["L"] else "DT(%d,%d)" % (c["tile"], c["subsweeps"])
-    return {"workload": "%s: RSOS N=%d, L=%d periodic, %d realizations per GPU, int32 heights, flat start, seed %d"
+    return {"workload": "%s: RSOS N=%d, L=%d periodic, %d realizations per GPU, flat start, seed %d"
                         % (name, c["N"], c["L"], c["R"], c["seed"]),
             "schedule": mode, "mcs_per_step": c["mcs_per_step"],
             "step": "rsos_advance(mcs_per_step) + rsos_width",
-            "l2": l2_note(c, info),
-            "parallelism": "replicas x%d (independent realizations, no collective)" % n_gpus}
+            "l2": L2_RULE,
+            "parallelism": "replicas x%d, no collective" % n_gpus}
 
 
 class ClockSampler(threading.Thread):
@@ -245,8 +255,7 @@ def run_reference(args):
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
             "config": config_dict(args, c, args.gpus),
-            "cpu_baseline": {"value": v / 1e9, "unit": UNIT, "cores": cores, "cpu_model": cpu_model(), "kind": "oracle",
-                             "sample": desc},
+            "cpu_baseline": {"value": v / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
             "e2e": {"value": v / 1e9, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -269,6 +278,20 @@ def alu_peak_attempts_per_s(sm_count, sm_mhz):
     return sm_count * 4 * 32 / cyc * sm_mhz * 1e6
 
 
+def engine_peak(info, sm_mhz):
+    """(peak attempts/s, where it comes from) for the update kernel of this engine, or (None, why).  The SASS count is the
+    attempt loop of the lane-per-tile kernel (THREAD engine); the other engines run other loops with other limiters
+    (barrier and claim rounds, vote and retry windows, bounded-draw rejection), so no instruction peak is claimed for
+    them: their `frac` is null and only the engine-independent fractions (22-instruction floor, int32-equivalent sweep)
+    are given."""
+    if info["engine"] == "thread":
+        return (alu_peak_attempts_per_s(info["sm_count"], sm_mhz),
+                "derived (DESIGN.md section 6): %d SMs x 4 schedulers x 32 lanes / 52.25 cycles per 32 attempts (alu pipe of the "
+                "SASS-counted loop of thread_dt_kernel<6,2,1>, profiles/r2_sass_attempt_loop.md) x %.0f MHz measured"
+                % (info["sm_count"], sm_mhz))
+    return None, "no SASS count for the %s engine's loop: peak not claimed" % info["engine"]
+
+
 def leg_config(name):
     """name = C1..C5, 'C3/N=2', 'C5/L=256' ... -> workload dict (utils/workloads.py holds the numbers)."""
     base, _, mod = name.partition("/")
@@ -287,9 +310,10 @@ def leg_config(name):
     return c
 
 
-def run_leg(pkg, torch, name, c, steps, warmup, engine, lanes, rank, world, local, barrier, do_e2e, dist):
-    """One timed leg: `warmup` untimed steps, then exactly `steps` steps between CUDA events on the kernels' stream
-    (barrier + synchronize on both sides, max over ranks), clocks sampled during the timed region."""
+def run_leg(pkg, torch, name, c, steps, warmup, engine, lanes, rank, world, local, barrier, do_e2e, dist, reps=1):
+    """One timed leg: `warmup` untimed steps, then `reps` timed regions of exactly `steps` steps each between CUDA events
+    on the kernels' stream (barrier + synchronize on both sides, max over ranks); the region with the median time is the
+    one reported.  Clocks are sampled during all timed regions."""
     import numpy as np
     L, N, R, mcs = c["L"], c["N"], c["R"], c["mcs_per_step"]
     stream = torch.cuda.Stream()
@@ -312,23 +336,28 @@ def run_leg(pkg, torch, name, c, steps, warmup, engine, lanes, rank, world, loca
         time.sleep(0.3)                                    # let nvidia-smi come up before the timed region
     g.kernel_time(True)                                    # per-advance CUDA events inside the library
     launches0 = g.info()["launches"]
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    if sampler:
-        sampler.mark()
-    e0.record(stream)
-    for _ in range(steps):
-        W2, hmean = step()
-    e1.record(stream)
-    barrier()
-    ms = e0.elapsed_time(e1)
+    reps = max(1, reps)
+    times = []
+    for rep in range(reps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        if sampler and rep == 0:
+            sampler.mark()
+        e0.record(stream)
+        for _ in range(steps):
+            W2, hmean = step()
+        e1.record(stream)
+        barrier()
+        t_rep = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([t_rep], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            t_rep = float(t.item())
+        times.append(t_rep)
     clocks = sampler.stop() if sampler else None
-    upd_ms, upd_launches = g.kernel_time(False)
-    launches = g.info()["launches"] - launches0
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    upd_ms, upd_launches = g.kernel_time(False)            # over all `reps` regions
+    launches = (g.info()["launches"] - launches0) // reps  # kernels launched inside ONE timed region of `steps` steps
+    ms = sorted(times)[len(times) // 2]
     value = att_step * steps * world / (ms * 1e-3)
 
     # ---- e2e: host buffers through the C ABI, H2D + D2H inside the timed region -----------------
@@ -361,33 +390,142 @@ def run_leg(pkg, torch, name, c, steps, warmup, engine, lanes, rank, world, loca
     # ---- roofline of the dominant kernel (the update kernel) ------------------------------------
     hbm, how = peaks()
     n_l = max(1, upd_launches)
-    per_launch_att = att_step * steps / n_l
+    per_launch_att = att_step * steps * reps / n_l
     avg_ms = upd_ms / n_l
-    kernel_rate = att_step * steps / (upd_ms * 1e-3)       # attempts/s of the update kernels alone
+    kernel_rate = att_step * steps * reps / (upd_ms * 1e-3)   # attempts/s of the update kernels alone
     sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
-    peak = alu_peak_attempts_per_s(info["sm_count"], sm_mhz)
+    peak, peak_src = engine_peak(info, sm_mhz)
     traffic, traffic_src = traffic_note(name, info)
     sweep_gbs = kernel_rate * BYTES_PER_ATTEMPT * c["subsweeps"] / 1e9 if info["mode"] == "DT" else None
-    roofline = {"bound": "alu", "achieved": kernel_rate / 1e9, "peak": peak / 1e9, "unit": "G attempts/s",
-                "frac": kernel_rate / peak, "traffic": traffic, "traffic_source": traffic_src,
-                "peak_source": "derived (DESIGN.md section 6): %d SMs x 4 schedulers x 32 lanes / 52.25 cycles per 32 attempts "
-                               "(alu pipe of the SASS-counted ideal loop, profiles/r2_sass_attempt_loop.md) x %.0f MHz measured"
-                               % (info["sm_count"], sm_mhz),
+    roofline = {"bound": "alu" if peak else "latency (serial chain; no instruction count for this engine)",
+                "achieved": kernel_rate / 1e9, "peak": peak / 1e9 if peak else None, "unit": "G attempts/s",
+                "frac": kernel_rate / peak if peak else None, "traffic": traffic, "traffic_source": traffic_src,
+                "peak_source": peak_src,
                 "kernel": "update kernel, engine=%s" % info["engine"],
                 "attempts_per_launch": per_launch_att, "avg_launch_ms": avg_ms, "update_launches": int(upd_launches),
-                "update_share_of_step": upd_ms / ms,
+                "update_share_of_step": upd_ms / sum(times),
                 "frac_of_survey_floor_22_instr": kernel_rate / (info["sm_count"] * 4 * 32 * sm_mhz * 1e6 / SURVEY_FLOOR_INSTR),
                 # north_star's other candidate, kept as a labelled int32-EQUIVALENT sweep rate: the packed working
                 # lattice moves far fewer bytes (see traffic), so this is not what binds
                 "int32_equiv_sweep": {"bytes_per_attempt": BYTES_PER_ATTEMPT * c["subsweeps"], "GBps": sweep_gbs,
                                       "hbm_peak_GBps": hbm, "peak_source": how,
                                       "frac": (sweep_gbs / hbm) if sweep_gbs else None}}
-    out = {"workload": name, "value": value / 1e9, "unit": UNIT, "steps": steps, "warmup": max(3, warmup),
-           "ms_per_step": ms / steps, "config": None, "engine": info, "clocks": clocks, "e2e": e2e,
+    out = {"workload": name, "value": value / 1e9, "unit": UNIT, "steps": steps, "warmup": max(3, warmup), "reps": reps,
+           "region_ms": times, "ms_per_step": ms / steps, "config": config_dict_for(name, c, world), "residency": l2_note(c, info),
+           "engine": info, "clocks": clocks, "e2e": e2e,
            "gpu_launches": int(launches), "roofline": roofline,
            "result_check": {"W2_mean": float(np.mean(W2)), "hmean_mean": float(np.mean(hmean)), "t_mcs": int(g.t)}}
     g.close()
     return out
+
+
+def run_seeds4(pkg, torch, c, steps, warmup, reps):
+    """BASELINE.json configs[1] as it is worded ("seeds 1..4"): the four 128-realization runs advance together, one
+    context per seed, each on its own stream, so that a colour pass has four times the tiles in flight.  A step = every
+    context's rsos_advance(mcs_per_step), then every context's rsos_width.  Device-timed from an event recorded while
+    all streams are idle to one recorded after the last width has synchronised its stream.  One GPU only."""
+    L, N, R, mcs = c["L"], c["N"], c["R"], c["mcs_per_step"]
+    seeds = (1, 2, 3, 4)
+    streams = [torch.cuda.Stream() for _ in seeds]
+    ctxs = [pkg.Rsos(L, N, R, sd, tile=c["tile"], subsweeps=c["subsweeps"], stream=st.cuda_stream) for sd, st in zip(seeds, streams)]
+
+    def step():
+        for g in ctxs:
+            g.advance(mcs)
+        return [g.width() for g in ctxs]
+
+    for _ in range(max(3, warmup)):
+        step()
+    times = []
+    for _ in range(max(1, reps)):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(streams[0])
+        for _ in range(steps):
+            step()
+        e1.record(streams[0])
+        torch.cuda.synchronize()
+        times.append(e0.elapsed_time(e1))
+    ms = sorted(times)[len(times) // 2]
+    launches = sum(g.info()["launches"] for g in ctxs)
+    for g in ctxs:
+        g.close()
+    att = workloads.attempts(L, R, mcs) * len(seeds) * steps
+    return {"workload": "C2 seeds 1..4", "value": att / (ms * 1e-3) / 1e9, "unit": UNIT, "steps": steps, "reps": reps,
+            "region_ms": times, "ms_per_step": ms / steps, "contexts": len(seeds), "launches_total": int(launches),
+            "what": "4 contexts (seeds 1..4) on 4 streams, advance all then width all"}
+
+
+def oracle_side_timings():
+    """The two other oracle timings SURVEY 8(d) / BASELINE.md section 3 list (G attempts/s each): a cut-down C4 (L = 32768,
+    one surface, 2 MCS) on all cores, and C1 in full on one thread.  The all-cores run comes first and names its thread
+    count: the oracle's thread setting is process-wide, so a one-thread run would otherwise carry over."""
+    from oracle import rsos_oracle
+    rsos_oracle.build()
+    out = {}
+    cores = os.cpu_count() or 1
+    c4 = workloads.CONFIGS["C4"]
+    try:
+        o = rsos_oracle.Oracle(c4["L"], c4["N"], 1, c4["seed"], tile=c4["tile"], subsweeps=c4["subsweeps"], threads=cores)
+        t0 = time.perf_counter()
+        o.advance(2)
+        o.width()
+        out["c4_cut_2mcs_allcores"] = workloads.attempts(c4["L"], 1, 2) / (time.perf_counter() - t0) / 1e9
+        o.close()
+    except (MemoryError, RuntimeError, ValueError) as e:   # 4 GiB of heights did not fit on this host
+        out["c4_cut_2mcs_allcores"] = None
+        out["c4_cut_error"] = str(e)[:80]
+    c1 = workloads.CONFIGS["C1"]
+    o = rsos_oracle.Oracle(c1["L"], c1["N"], c1["R"], c1["seed"], tile=c1["tile"], subsweeps=c1["subsweeps"], threads=1)
+    t0 = time.perf_counter()
+    o.advance(c1["mcs"])
+    o.width()
+    out["c1_full_1thread"] = workloads.attempts(c1["L"], c1["R"], c1["mcs"]) / (time.perf_counter() - t0) / 1e9
+    o.close()
+    return out
+
+
+def r6(x):
+    """Six significant digits: keeps the final line short."""
+    return float("%.6g" % x) if isinstance(x, float) else x
+
+
+def make_line(c, world, steps, warmup, head, cpu=None, c4=None, seeds4=None, legs_file=None):
+    """The ONE final stdout line: the headline leg `head` (a run_leg record) reduced to the keys the contract names,
+    plus compact side numbers.  Must stay below MAX_LINE_BYTES; optional parts are dropped, last first, if it does not."""
+    rf, ie = head["roofline"], head["roofline"]["int32_equiv_sweep"]
+    ck = head["clocks"] or {}
+    line = {"metric": METRIC, "value": r6(head["value"]), "unit": UNIT, "n_gpus": world, "steps": steps,
+            "warmup": max(3, warmup), "ms_per_step": r6(head["ms_per_step"]), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int32", "data": "synthetic", "config": head["config"], "reps": head["reps"],
+            "clocks": {k: ck.get(k) for k in ("sm_mhz", "sm_max_mhz", "reasons", "samples")},
+            "e2e": None if not head["e2e"] else {k: r6(head["e2e"][k]) for k in ("value", "unit", "h2d_bytes_per_step", "d2h_bytes_per_step")},
+            "gpu_launches": head["gpu_launches"],
+            "roofline": {"bound": rf["bound"], "achieved": r6(rf["achieved"]), "peak": r6(rf["peak"]), "unit": rf["unit"],
+                         "frac": r6(rf["frac"]), "traffic": rf["traffic"],
+                         "kernel": "%s engine, %d lanes/tile, %d bits/site" % (head["engine"]["engine"], head["engine"].get("lanes", 0),
+                                                                              head["engine"].get("packed_bits", 0)),
+                         "avg_launch_ms": r6(rf["avg_launch_ms"]), "attempts_per_launch": int(rf["attempts_per_launch"]),
+                         "update_share_of_step": r6(rf["update_share_of_step"]),
+                         "frac_hbm_int32_equiv": r6(ie["frac"]),
+                         "frac_of_survey_floor_22_instr": r6(rf["frac_of_survey_floor_22_instr"]),
+                         "peak_source": "DESIGN.md 6"},
+            "cpu_baseline": None if not cpu else {k: r6(v) for k, v in cpu.items()}}
+    if c4:
+        line["c4"] = {"value": r6(c4["value"]), "kernel": r6(c4["roofline"]["achieved"]), "frac": r6(c4["roofline"]["frac"]),
+                      "frac_hbm_int32_equiv": r6(c4["roofline"]["int32_equiv_sweep"]["frac"]),
+                      "e2e": r6(c4["e2e"]["value"]) if c4.get("e2e") else None}
+    if seeds4:
+        line["c2_seeds4"] = {"value": r6(seeds4["value"]), "ms_per_step": r6(seeds4["ms_per_step"]), "what": "4 contexts, 4 streams"}
+    if legs_file:
+        line["legs_file"] = os.path.basename(legs_file)
+    for drop in ("legs_file", "c2_seeds4", "c4"):
+        if len(json.dumps(line)) < MAX_LINE_BYTES:
+            break
+        line.pop(drop, None)
+    if len(json.dumps(line)) >= MAX_LINE_BYTES:
+        raise RuntimeError("bench.py: final line is %d bytes (limit %d)" % (len(json.dumps(line)), MAX_LINE_BYTES))
+    return line
 
 
 def run_b200(args):
@@ -416,19 +554,18 @@ def run_b200(args):
     c = workload(args)
     engine = {"auto": 0, "simple": 1, "warp": 2, "onchip": 3, "thread": 4, "resident": 5, "fine": 6, "level": 8}[args.engine]
     head = run_leg(pkg, torch, args.workload, c, args.steps, args.warmup, engine, args.lanes, rank, world, local, barrier,
-                   not args.no_e2e, dist)
+                   not args.no_e2e, dist, reps=args.reps)
 
-    # ---- the other BASELINE configs, same fields, fewer steps (one GPU only) -------------------------
-    extra = {}
+    # ---- side legs (one GPU only): full records go to the side file, two compact numbers to the final line ----------
+    legs, seeds4 = {}, None
     if world == 1 and not args.no_extra:
-        for name in EXTRA_LEGS:
+        for name in (EXTRA_LEGS if args.all_legs else DEFAULT_LEGS):
             if name == args.workload:
                 continue
-            ce = leg_config(name)
-            leg = run_leg(pkg, torch, name, ce, args.extra_steps, 3, 0, 0, rank, world, local, barrier,
-                          not args.no_e2e, dist)
-            leg["config"] = config_dict_for(name, ce, 1, leg["engine"])
-            extra[name] = leg
+            legs[name] = run_leg(pkg, torch, name, leg_config(name), args.extra_steps, 3, 0, 0, rank, world, local, barrier,
+                                 not args.no_e2e, dist, reps=args.reps)
+        if args.workload == "C2":
+            seeds4 = run_seeds4(pkg, torch, c, max(1, args.steps // 2), 3, args.reps)
 
     if rank != 0:
         if world > 1:
@@ -438,13 +575,16 @@ def run_b200(args):
     cpu = None
     if not args.no_cpu_baseline and world == 1:
         v, cores, desc, _ = oracle_sample(c, args.cpu_seconds)
-        cpu = {"value": v / 1e9, "unit": UNIT, "cores": cores, "cpu_model": cpu_model(), "kind": "oracle", "sample": desc}
+        cpu = {"value": v / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+        cpu.update(oracle_side_timings())
 
-    line = {"metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(3, args.warmup), "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "int32", "data": "synthetic", "config": config_dict(args, c, world, head["engine"]),
-            "engine": head["engine"], "clocks": head["clocks"], "e2e": head["e2e"], "gpu_launches": head["gpu_launches"],
-            "roofline": head["roofline"], "cpu_baseline": cpu, "result_check": head["result_check"], "extra": extra}
+    try:
+        with open(args.legs_file, "w") as f:
+            json.dump({"headline": head, "legs": legs, "c2_seeds4": seeds4, "cpu_baseline": cpu, "cpu_model": cpu_model()}, f, indent=1)
+        legs_file = args.legs_file
+    except OSError:
+        legs_file = None
+    line = make_line(c, world, args.steps, args.warmup, head, cpu, legs.get("C4"), seeds4, legs_file)
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
