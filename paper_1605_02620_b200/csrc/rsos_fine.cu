@@ -98,10 +98,15 @@ __global__ void __launch_bounds__(1024) fine_dt_kernel(Params p, uint32_t t0, ui
     const uint32_t latb = (uint32_t)__cvta_generic_to_shared(smem + (live ? rs : 0u) * sh.lat_words);
     const uint32_t A = (C * C) / p.K, N = p.N;
     const uint32_t a_ = n % half, b_ = n / half;
+    // A launch covers up to 2^36 attempts (rsos_api.cu) and on a small lattice with few realizations a thread owns a large
+    // share of them: the count of one sub-sweep (at most a few hundred) is kept in 32 bits and folded into 64 after it.
     uint32_t nacc = 0;
+    unsigned long long nacc_total = 0;
 
     for (uint32_t m = 0; m < mcs; ++m)
     for (uint32_t k = 0; k < p.K; ++k) {
+        nacc_total += nacc;
+        nacc = 0;
         const uint32_t u = (t0 + m) * p.K + k;
         uint32_t ox = 0, oy = 0;
         if (live) draw_origin(p, u, rg, ox, oy);
@@ -164,7 +169,8 @@ __global__ void __launch_bounds__(1024) fine_dt_kernel(Params p, uint32_t t0, ui
             else dst[i] = gather8(smem[2u * i]) | (gather8(smem[2u * i + 1u]) << 16);
         }
     }
-    if (live && nacc) atomicAdd(p.accepted + rl, (unsigned long long)nacc);
+    nacc_total += nacc;
+    if (live && nacc_total) atomicAdd(p.accepted + rl, nacc_total);
 }
 
 // =============================================================================================

@@ -333,8 +333,12 @@ __global__ void __launch_bounds__(512) resident_dt_kernel(Params p, uint32_t t0,
             pko[i] = v;
         }
     }
-    const uint32_t tot = __reduce_add_sync(FULL, nacc);
-    if (lane == 0 && tot) atomicAdd(p.accepted + rl, (unsigned long long)tot);
+    // A launch covers up to 2^36 attempts (rsos_api.cu) and a warp may own all of them (one tile per colour pass, R = 1):
+    // a lane's count stays below 2^31, the warp's total does not fit 32 bits -- sum the lanes in 64.
+    unsigned long long tot = nacc;
+#pragma unroll
+    for (int o = 16; o; o >>= 1) tot += __shfl_xor_sync(FULL, tot, o);
+    if (lane == 0 && tot) atomicAdd(p.accepted + rl, tot);
 }
 
 // =============================================================================================
