@@ -34,7 +34,8 @@ __global__ void __launch_bounds__(RED_THREADS) sums_kernel(const int32_t *__rest
         }
     } else {
         const int32_t *src = h + (size_t)r * n;
-        for (uint32_t i = blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += gridDim.x * RED_THREADS) {
+        // 64-bit index: at L = 65535 (the one odd L this large) n = 4294836225 and a 32-bit i + stride would wrap below n
+        for (uint64_t i = (uint64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n; i += (uint64_t)gridDim.x * RED_THREADS) {
             const int v = __ldg(src + i);
             s1 += (long long)v;
             s2 += (unsigned long long)((long long)v * v);
@@ -130,7 +131,8 @@ __global__ void __launch_bounds__(RED_THREADS) moments_kernel(const int32_t *__r
         }
     } else {
         const int32_t *src = h + (size_t)r * n4;
-        for (uint32_t i = blockIdx.x * RED_THREADS + threadIdx.x; i < n4; i += gridDim.x * RED_THREADS) add(__ldg(src + i));
+        for (uint64_t i = (uint64_t)blockIdx.x * RED_THREADS + threadIdx.x; i < n4; i += (uint64_t)gridDim.x * RED_THREADS)
+            add(__ldg(src + i));                           // 64-bit index, as in sums_kernel
     }
     for (int o = 16; o; o >>= 1)
 #pragma unroll

@@ -114,6 +114,7 @@ __device__ __forceinline__ void general_dt_pass(const Params &p, uint32_t u, uin
 // than the (2S)^2 attempts a tile has), so the byte delta is the true one.
 // ---------------------------------------------------------------------------------------------
 constexpr uint32_t GW_NT = 16;
+constexpr uint32_t GW_MAX_COLS = 128;      // staging and write-back move 4 chunks of 32 lanes per window row: columns 0..127
 
 __global__ void __launch_bounds__(32) general_window_kernel(Params p, uint32_t u, uint32_t colour, uint32_t pww, uint32_t nrows)
 {
@@ -247,6 +248,8 @@ static bool general_window_shape(const Params &p, uint32_t *pww, uint32_t *nrows
 {
     if (!p.general || !p.T || p.N > 7) return false;
     const uint32_t wmax = (p.L + p.T - 1) / p.T;                       // ceil(L / T): the larger of the two tile sizes
+    if (wmax + 2 > GW_MAX_COLS) return false;                          // wider windows: simple_dt_kernel (the shared-memory
+                                                                       // cap below is tighter today; this keeps it explicit)
     *pww = (wmax + 2 + 3) / 4;
     *nrows = wmax + 2;
     *smem = (size_t)*pww * *nrows * GW_NT * 4;

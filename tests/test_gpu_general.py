@@ -35,6 +35,8 @@ def _same(g, o, R):
     (150, 9, 2, 64, 1, 3, 0),        # N > 7: thread per tile in global memory (the windowed kernel needs N <= 7)
     (1000, 7, 35, 64, 2, 2, 3),      # T = 14: 49 tiles per pass and realization, ragged last warp of 16 tiles, N = 7
     (300, 1, 2, 128, 1, 2, 0),       # T = 2, tiles of 150 x 150: windows too large for shared memory -> global path
+    (220, 1, 2, 64, 1, 3, 0),        # T = 2, tiles of 110 x 110: the widest windows the shared-memory kernel takes
+    (255, 2, 2, 64, 1, 3, 1),        # T = 2, tiles of 127 / 128: window rows of 130 columns exceed the 128 the kernel stages
     (45, 1, 4, 64, 1, 12, 0),        # RSG (2S > L), odd L
     (6, 1, 5, 64, 1, 40, 2),         # RSG, tiny
 ])
