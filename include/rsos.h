@@ -53,7 +53,9 @@ enum {
                              /* DT mode: FINE when it applies (tile 8 or 16, L <= 512), else      */
                              /* THREAD when it applies and one colour pass has at least           */
                              /* RSOS_THREAD_MIN_TILES active tiles, else RESIDENT when it         */
-                             /* applies, else WARP, else SIMPLE.  L not a power of two: SIMPLE.   */
+                             /* applies, else WARP, else SIMPLE.  L not a power of two: THREAD    */
+                             /* (packed lattice, one lane per tile) under the condition stated    */
+                             /* at rsos_init, else SIMPLE.                                        */
                              /* rsos_plan() tells what a given set of arguments selects.          */
     RSOS_ENGINE_SIMPLE = 1,  /* one thread per active tile, heights in global memory (slow;       */
                              /* the literal loop nest of D:2, kept as an on-device cross-check;   */
@@ -100,7 +102,8 @@ typedef struct rsos_opts {
                           /* packed lattice (D:5) and this buffer is brought up to date only by   */
                           /* rsos_get_heights, rsos_moments, rsos_set_state, rsos_device_heights. */
     void    *stream;      /* cudaStream_t to enqueue on; NULL = the legacy default stream         */
-    int32_t  device;      /* CUDA device ordinal + 1; 0 = the current device                      */
+    int32_t  device;      /* CUDA device ordinal + 1; 0 = the current device (so that a zeroed    */
+                          /* struct means "all defaults"; SURVEY 8(b) wrote -1 = current instead)  */
     uint32_t lanes;       /* THREAD engine: lanes that share one tile, 1, 2, 4 or 8 (8 * lanes must not   */
                           /* exceed tile^2 / subsweeps); 0 = chosen from the number of tiles per colour   */
                           /* pass (D:4).  Does not change the result.                                     */
