@@ -10,6 +10,13 @@ Two kinds of check, both bit-exact (integers):
              must agree.  With the exact prefixes this covers the run by induction on the sampled steps, and it is
              the test of the packed / mod-64 on-chip formats and of the anchor division far from the flat start.
 No expected value comes from the CUDA path.
+
+Tiers: A = the oracle runs the whole config; B = a full-oracle prefix of >= 16 MCS, snapshot induction at
+>= 8 measurement times and, for configs with many realizations, >= 2 single realizations followed by the oracle for the
+COMPLETE run (sums compared at every measurement time, heights at the end).  The `tier_b` tests below bring configs[1],
+[2], [3] and [4] to B (configs[4] at L = 64 and 128 has 16 complete realizations per (L, N); at L = 256 and 512 a complete
+realization costs minutes of oracle time and is left out, so those two sizes hold B's induction and prefix parts only).
+configs[0] is at A in test_gpu_parity.py.
 """
 import numpy as np
 import pytest
@@ -45,6 +52,135 @@ def _check_realization(g, gs, oracle_mod, cfg, r, t0, mcs, state=None):
     assert bad.size == 0, "r=%d heights differ at %d sites, first %s" % (r, len(bad), bad[:4].tolist())
 
 
+def _spread(seq, n):
+    """n entries of seq, first and last included, evenly spread by index."""
+    return [seq[(i * (len(seq) - 1)) // (n - 1)] for i in range(n)]
+
+
+def _tier_b(rsos, oracle_mod, c, complete, induct, times, induct_times, expect_engine, oracle_R=1):
+    """The GPU runs the FULL config c (engine = auto) through `times` (sorted measurement times, t_max last).
+      - `complete`: first realizations of oracle runs (oracle_R consecutive realizations each) that follow the whole run from
+        the flat start and are compared at every entry of `times` (S1, S2, accepted) and at the end (heights);
+      - at every t in `induct_times` the GPU state of the realizations in `induct` goes to a fresh oracle (set_state; t enters
+        the Philox counter), both sides advance one MCS and must agree in sums and in every height."""
+    g = rsos.Rsos(c["L"], c["N"], c["R"], c["seed"], tile=c["tile"], subsweeps=c["subsweeps"])
+    assert g.info()["engine"] in expect_engine, g.info()
+    kw = dict(tile=c["tile"], subsweeps=c["subsweeps"])
+    stops = sorted(set(times) | set(induct_times) | {t + 1 for t in induct_times})
+    assert stops[-1] == times[-1] == c["mcs"]
+    sums_at, pending = {}, {}
+    for t in stops:
+        g.advance(t - g.t)
+        gs = g.sums()
+        assert (gs[0] == gs[2]).all(), "t=%d: sum h != accepted" % t
+        if t in times:
+            sums_at[t] = gs
+        for r, o in pending.pop(t - 1, []):                # oracles started one MCS ago from the GPU's state
+            os1, os2, oacc = o.sums()
+            assert (gs[0][r], gs[1][r], gs[2][r]) == (os1[0], os2[0], oacc[0]), "induction t=%d r=%d sums" % (t - 1, r)
+            assert np.array_equal(g.heights(r, 1), o.heights()), "induction t=%d r=%d heights" % (t - 1, r)
+            o.close()
+        if t in induct_times:
+            pending[t] = []
+            for r in induct:
+                o = oracle_mod.Oracle(c["L"], c["N"], 1, c["seed"], first_real=r, **kw)
+                o.set_state(g.heights(r, 1), t, gs[2][r:r + 1].copy())
+                o.advance(1)
+                pending[t].append((r, o))
+    assert not pending and g.t == c["mcs"]
+    for r0 in complete:                                    # complete single realizations, flat start to t_max
+        o = oracle_mod.Oracle(c["L"], c["N"], oracle_R, c["seed"], first_real=r0, **kw)
+        for t in times:
+            o.advance(t - o.t)
+            for a, b in zip(sums_at[t], o.sums()):
+                assert (a[r0:r0 + oracle_R] == b).all(), "complete run r0=%d t=%d" % (r0, t)
+        assert np.array_equal(g.heights(r0, oracle_R), o.heights()), "complete run r0=%d final heights" % r0
+        o.close()
+    g.close()
+
+
+def _measurement_times(t_max, prefix=16):
+    """The config's 64 log-spaced times plus every MCS of the first `prefix` (the full-oracle prefix of tier B)."""
+    return sorted(set(workloads.log_spaced_times(t_max)) | set(range(1, prefix + 1)))
+
+
+def _induction_times(t_max):
+    """8 times: 7 of the log-spaced measurement times beyond the prefix, spread over the run, and the last MCS of the run."""
+    return _spread([t for t in workloads.log_spaced_times(t_max) if 16 < t < t_max - 1], 7) + [t_max - 1]
+
+
+def test_c2_tier_b(rsos, oracle_mod):
+    """configs[1] in full on the GPU (128 realizations, 10^4 MCS, the 4-lanes-per-tile launch bench.py times).  Realizations
+    0 and 127 are followed by the oracle for the WHOLE run (1.05e10 attempts each) and compared at the 57 log-spaced times
+    and at every MCS up to 16; realizations 17 and 100 are handed over at 8 measurement times."""
+    c = dict(workloads.CONFIGS["C2"])
+    times = _measurement_times(c["mcs"])
+    induct_times = _induction_times(c["mcs"])
+    _tier_b(rsos, oracle_mod, c, complete=(0, 127), induct=(17, 100), times=times, induct_times=induct_times,
+            expect_engine=("thread",))
+
+
+@pytest.mark.parametrize("N", [1, 2, 3, 4])
+def test_c3_tier_b(rsos, oracle_mod, N):
+    """configs[2] in full on the GPU at every N (64 realizations, 5000 MCS): one complete oracle realization per N (four
+    over the config, 2.1e10 attempts each), two realizations handed over at 8 measurement times."""
+    c = dict(workloads.CONFIGS["C3"])
+    c["N"] = N
+    times = _measurement_times(c["mcs"])
+    induct_times = _induction_times(c["mcs"])
+    _tier_b(rsos, oracle_mod, c, complete=((0, 21, 42, 63)[N - 1],), induct=(5, 62), times=times, induct_times=induct_times,
+            expect_engine=("thread",))
+
+
+@pytest.mark.parametrize("N", [1, 2])
+@pytest.mark.parametrize("L", [64, 128, 256, 512])
+def test_c5_tier_b(rsos, oracle_mod, L, N):
+    """configs[4] on the GPU at the config's own R, up to t = 20 L^1.6 (0.8 of it at L = 512): two realizations handed over at 8 times
+    spread over the run (the last ones inside the stationary measurement window, |h| up to ~1e5 at L = 512); at L = 64 and
+    128 sixteen consecutive realizations are followed by the oracle for the complete run."""
+    c = _c5(L, N)
+    t_full = c["mcs"]
+    if L == 512:
+        c["mcs"] = int(0.8 * t_full)                        # 7e12 attempts in full: stop a little inside the measurement window
+    times = _measurement_times(c["mcs"])
+    induct_times = _induction_times(c["mcs"])
+    assert induct_times[-1] > 0.75 * t_full                 # inside the final 25 % the config averages over
+    complete = (c["R"] // 2,) if L <= 128 else ()
+    _tier_b(rsos, oracle_mod, c, complete=complete, induct=(1, c["R"] - 2), times=times, induct_times=induct_times,
+            expect_engine=("onchip", "resident"), oracle_R=16)
+
+
+def test_c4_tier_b(rsos, oracle_mod):
+    """configs[3]: the whole 2^30-site surface.  Prefix: the oracle follows it from the flat start for 16 MCS (sums every MCS,
+    every height at t = 16).  Induction: at 8 of the config's log-spaced times up to t = 1999 the whole surface goes to the
+    oracle, both sides advance one MCS, sums and all 2^30 heights must agree."""
+    c = dict(workloads.CONFIGS["C4"])
+    L = c["L"]
+    g = rsos.Rsos(L, c["N"], 1, c["seed"], tile=c["tile"], subsweeps=c["subsweeps"])
+    assert g.info()["engine"] == "thread"
+    o = oracle_mod.Oracle(L, c["N"], 1, c["seed"], tile=c["tile"], subsweeps=c["subsweeps"])
+    for t in range(1, 17):
+        g.advance(1)
+        o.advance(1)
+        assert all((a == b).all() for a, b in zip(g.sums(), o.sums())), "prefix t=%d" % t
+    assert np.array_equal(g.heights(), o.heights()), "prefix heights at t = 16"
+    induct_times = _induction_times(c["mcs"])
+    for t in induct_times:
+        g.advance(t - g.t)
+        h0 = g.heights()
+        o.set_state(h0, t, g.sums()[2])
+        del h0
+        g.advance(1)
+        o.advance(1)
+        assert all((a == b).all() for a, b in zip(g.sums(), o.sums())), "induction t=%d sums" % t
+        hg = g.heights()
+        assert np.array_equal(hg, o.heights()), "induction t=%d heights" % t
+        del hg
+    assert g.t == c["mcs"]
+    g.close()
+    o.close()
+
+
 def _c5(L, N):
     c = dict(workloads.CONFIGS["C5"])
     c.update(L=L, N=N, R=workloads.c5_realizations(L), mcs=workloads.c5_mcs(L))
@@ -69,34 +205,6 @@ def test_c5_full_size_prefix(rsos, oracle_mod, L, N):
     g.close()
 
 
-@pytest.mark.parametrize("N", [1, 2])
-@pytest.mark.parametrize("L", [64, 128, 256, 512])
-def test_c5_full_size_saturated_induction(rsos, oracle_mod, L, N):
-    """configs[4] at t0 = 0.75 * t_max (inside the config's measurement window, the stationary regime): two
-    realizations go to the oracle, both sides advance 2 MCS.  Heights are ~ 0.3 * t0 (up to ~1e5 at L = 512)."""
-    c = _c5(L, N)
-    t0 = int(0.75 * c["mcs"])
-    g = rsos.Rsos(L, N, c["R"], c["seed"], tile=c["tile"], subsweeps=c["subsweeps"])
-    g.advance(t0)
-    s1, s2, acc = g.sums()
-    assert (s1 == acc).all()
-    w2, hm = g.width()
-    assert hm.min() > 0.2 * t0                              # grown far from the flat start
-    assert w2.mean() > 0.08 * L ** 0.78, w2.mean()          # loose: a saturated width ~ 0.118 L^(2 alpha) at N = 1, more at N = 2
-    picks = (1, c["R"] - 2)
-    states = {}
-    for r in picks:
-        h0 = g.heights(r, 1)
-        for ax in (0, 1):
-            assert np.abs(h0[0] - np.roll(h0[0], 1, axis=ax)).max() <= N      # Eq. (6), periodic
-        states[r] = (h0, acc[r:r + 1].copy())
-    g.advance(2)
-    gs = g.sums()
-    for r in picks:
-        _check_realization(g, gs, oracle_mod, c, r, t0, 2, states[r])
-    g.close()
-
-
 @pytest.mark.parametrize("N", [2, 3])
 def test_c3_full_size_sampled_realizations_n23(rsos, oracle_mod, N):
     """configs[2] at N = 2 and 3 (N = 1 and 4 are in test_gpu_parity.py): 16384 tiles per pass, 4-bit sites."""
@@ -110,64 +218,6 @@ def test_c3_full_size_sampled_realizations_n23(rsos, oracle_mod, N):
     for r in (0, 31, 63):
         _check_realization(g, gs, oracle_mod, c, r, 0, 3)
     g.close()
-
-
-@pytest.mark.parametrize("N", [1, 2, 3, 4])
-def test_c3_full_size_late_induction(rsos, oracle_mod, N):
-    """configs[2] at its end: t0 = 4998, two realizations handed to the oracle, 2 MCS to t = 5000."""
-    c = dict(workloads.CONFIGS["C3"])
-    c["N"] = N
-    t0 = c["mcs"] - 2
-    g = rsos.Rsos(c["L"], N, c["R"], c["seed"], tile=c["tile"], subsweeps=c["subsweeps"])
-    g.advance(t0)
-    acc = g.sums()[2]
-    states = {r: (g.heights(r, 1), acc[r:r + 1].copy()) for r in (5, 62)}
-    g.advance(2)
-    assert g.t == c["mcs"]
-    gs = g.sums()
-    for r, st in states.items():
-        _check_realization(g, gs, oracle_mod, c, r, t0, 2, st)
-    g.close()
-
-
-def test_c2_full_size_induction_at_the_end(rsos, oracle_mod):
-    """configs[1] at its end: t0 = 9998 of 10^4 MCS (all 128 realizations on the GPU), realizations 0, 64, 127."""
-    c = dict(workloads.CONFIGS["C2"])
-    t0 = c["mcs"] - 2
-    g = rsos.Rsos(c["L"], c["N"], c["R"], c["seed"], tile=c["tile"], subsweeps=c["subsweeps"])
-    g.advance(t0)
-    acc = g.sums()[2]
-    states = {r: (g.heights(r, 1), acc[r:r + 1].copy()) for r in (0, 64, 127)}
-    for st in states.values():
-        assert st[0].max() - st[0].min() > 12
-    g.advance(2)
-    assert g.t == c["mcs"]
-    gs = g.sums()
-    for r, st in states.items():
-        _check_realization(g, gs, oracle_mod, c, r, t0, 2, st)
-    g.close()
-
-
-def test_c4_full_size_induction_at_the_end(rsos, oracle_mod):
-    """configs[3] at its end: the whole 2^30-site surface at t0 = 1999 goes to the oracle; 1 MCS to t = 2000."""
-    c = dict(workloads.CONFIGS["C4"])
-    L, t0 = c["L"], c["mcs"] - 1
-    g = rsos.Rsos(L, c["N"], 1, c["seed"], tile=c["tile"], subsweeps=c["subsweeps"])
-    g.advance(t0)
-    h0 = g.heights()
-    acc = g.sums()[2]
-    o = oracle_mod.Oracle(L, c["N"], 1, c["seed"], tile=c["tile"], subsweeps=c["subsweeps"])
-    o.set_state(h0, t0, acc)
-    del h0
-    g.advance(1)
-    o.advance(1)
-    assert g.t == c["mcs"]
-    assert all((a == b).all() for a, b in zip(g.sums(), o.sums()))
-    hg = g.heights()
-    g.close()
-    ho = o.heights()
-    o.close()
-    assert np.array_equal(hg, ho)
 
 
 @pytest.mark.parametrize("L,N,R,S,K,mcs", [(256, 3, 3, 64, 1, 6), (64, 1, 5, 64, 1, 40), (128, 2, 2, 64, 4, 9)])
