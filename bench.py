@@ -71,7 +71,7 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="skip the side legs (C4, C2 with seeds 1..4)")
     ap.add_argument("--all-legs", action="store_true", help="also time C3, C3/N=2, C5 (L=64..512), C1 and X1 (side file only)")
-    ap.add_argument("--extra-steps", type=int, default=5, help="timed steps of each side leg")
+    ap.add_argument("--extra-steps", type=int, default=15, help="timed steps of each side leg (15: >= 10 clock samples per leg)")
     ap.add_argument("--reps", type=int, default=3, help="timed regions of --steps steps each; the median is reported")
     ap.add_argument("--legs-file", default=os.path.join(ROOT, "bench_legs.json"), help="where the full per-leg records go")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")

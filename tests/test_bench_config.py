@@ -95,3 +95,19 @@ def test_no_instruction_peak_is_claimed_for_other_engines(bench):
         assert peak is None and eng in src
     peak, _ = bench.engine_peak({"engine": "thread", "sm_count": 148}, 1965.0)
     assert peak == pytest.approx(712.4e9, rel=1e-3)
+
+
+def test_selfcheck_cases_resolve_to_their_engines():
+    """paper_1605_02620_b200.selfcheck: every case of the engine tour selects the engine it names (host-only planning)."""
+    import paper_1605_02620_b200 as pkg
+    from paper_1605_02620_b200 import selfcheck
+    seen = set()
+    for name, L, N, R, kw, engine in selfcheck.CASES:
+        pl = pkg.plan(L, N, R, **kw)
+        assert pl["engine"] == engine, (name, pl)
+        if "lanes" in kw:
+            assert pl["lanes"] == kw["lanes"], name
+        if "cluster" in kw:
+            assert pl["cluster"] == kw["cluster"], name
+        seen.add(engine)
+    assert seen == {"thread", "resident", "fine", "level", "onchip", "multi", "warp", "simple"}
