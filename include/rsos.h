@@ -147,7 +147,10 @@ int rsos_init(rsos_ctx **ctx, uint32_t L, uint32_t N, uint32_t R, uint64_t seed,
 /*
  * rsos_advance -- advance every realization by `mcs` Monte-Carlo steps of the schedule D:2
  * (P:61-63 rule, P:77 decomposition): t += mcs.  Asynchronous: kernels are enqueued on the
- * context's stream and the call returns.  mcs = 0 is a no-op.
+ * context's stream and the call returns.  mcs = 0 is a no-op.  Contexts on different streams run concurrently:
+ * when one context has few tiles per colour pass (BASELINE configs[1]: 8192), calling rsos_advance on several
+ * contexts (one per seed, a stream each) before reading any of them back fills the GPU (D:11: 304 against 197 G
+ * attempts/s for the four seeds of configs[1]).
  * Errors: RSOS_ERANGE if (t + mcs) * K >= 2^32 (nothing is enqueued), RSOS_ECUDA.
  */
 int rsos_advance(rsos_ctx *ctx, uint64_t mcs);

@@ -2,7 +2,7 @@
 SURVEY section 5: per-measurement rows; Eq. 10).
 
     python -m paper_1605_02620_b200.timeseries C2 [--out c2.jsonl] [--schedule log64|eq10|every] [--tmax T]
-                                                  [--moments] [--R r] [--seed s]
+                                                  [--moments] [--R r] [--seed s] [--seeds 1,2,3,4]
 
 One JSONL row per measurement time and realization: {"t", "r", "S1", "S2", "accepted"} (exact integers, Eq. 2 follows
 from them: W2 = (L^2 S2 - S1^2) / L^4), with "phi2", "phi3", "phi4" (Eq. 13) added by --moments; a header row names
@@ -61,6 +61,39 @@ def run(pkg, cfg, times, out=None, moments=False, engine=0):
     return list(times), np.array(W2s), np.array(hms)
 
 
+def run_seeds(pkg, cfg, seeds, times, out=None):
+    """BASELINE.json configs[1] asks for "seeds 1..4": the same workload once per seed.  This runs them TOGETHER -- one
+    context per seed, each on its own CUDA stream; rsos_advance only enqueues, so all contexts' kernels are in flight at once
+    -- which is how a config with few tiles per colour pass fills the GPU (C2: 304 against 197 G attempts/s on a B200,
+    DESIGN.md section 11).  Each seed's run is the same pure function of (seed, r, ...) as a lone run; only the wall time
+    changes.  Returns (times, W2[len(seeds), len(times), R]); JSONL rows carry a "seed" field."""
+    import torch
+    streams = [torch.cuda.Stream() for _ in seeds]
+    ctxs = [pkg.Rsos(cfg["L"], cfg["N"], cfg["R"], sd, tile=cfg["tile"], subsweeps=cfg["subsweeps"],
+                     first_real=cfg.get("first_real", 0), stream=st.cuda_stream) for sd, st in zip(seeds, streams)]
+    if out is not None:
+        out.write(json.dumps({"header": True, "config": {k: cfg[k] for k in ("L", "N", "R", "tile", "subsweeps")},
+                              "seeds": list(seeds), "engine": ctxs[0].info()["engine"]}) + "\n")
+    W2s, t = [[] for _ in seeds], 0
+    for tm in times:
+        tm = int(tm)
+        if tm < t:
+            raise ValueError("measurement times must ascend")
+        for g in ctxs:
+            g.advance(tm - t)                              # asynchronous: enqueued on every stream before any read-back
+        t = tm
+        for i, (sd, g) in enumerate(zip(seeds, ctxs)):
+            S1, S2, acc = g.sums()
+            W2s[i].append(g.width()[0])
+            if out is not None:
+                for r in range(cfg["R"]):
+                    out.write(json.dumps({"t": t, "seed": int(sd), "r": cfg.get("first_real", 0) + r, "S1": int(S1[r]),
+                                          "S2": int(S2[r]), "accepted": int(acc[r])}) + "\n")
+    for g in ctxs:
+        g.close()
+    return list(times), np.array(W2s)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("workload", help="C1..C5 (paper_1605_02620_b200/utils/workloads.py)")
@@ -70,6 +103,7 @@ def main():
     ap.add_argument("--R", type=int, default=0)
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--moments", action="store_true")
+    ap.add_argument("--seeds", default="", help="e.g. 1,2,3,4: run these seeds together, one context and stream each")
     a = ap.parse_args()
     import paper_1605_02620_b200 as pkg
     cfg = dict(workloads.CONFIGS[a.workload])
@@ -81,6 +115,20 @@ def main():
     schedule = a.schedule or ("every" if a.workload == "C1" else "log64")
     times = measurement_times(schedule, t_max)
     f = open(a.out, "w") if a.out else None
+    if a.seeds:
+        seeds = [int(x) for x in a.seeds.split(",")]
+        try:
+            ts, W2 = run_seeds(pkg, cfg, seeds, times, out=f)
+        finally:
+            if f:
+                f.close()
+        w2m = W2.mean(axis=(0, 2))                           # over seeds and realizations
+        bt, be = analysis.beta_eff(ts, w2m)
+        json.dump({"workload": a.workload, "schedule": schedule, "seeds": seeds, "times": ts, "W2_mean": w2m.tolist(),
+                   "W2_stderr": [analysis.standard_error(W2[:, i, :].ravel()) for i in range(len(ts))],
+                   "beta_eff": {"t": bt.tolist(), "beta": be.tolist()}}, sys.stdout)
+        sys.stdout.write("\n")
+        return
     try:
         ts, W2, hm = run(pkg, cfg, times, out=f, moments=a.moments)
     finally:

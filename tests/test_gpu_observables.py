@@ -55,6 +55,30 @@ def test_timeseries_rows_equal_oracle(rsos, oracle_mod, cfg, times):
     o.close()
 
 
+def test_seeds_run_together_equal_the_oracle_seed_by_seed(rsos, oracle_mod):
+    """timeseries.run_seeds: several seeds advance together (a context and a stream each, as bench.py's c2_seeds4 leg does);
+    every seed's rows must be what the oracle gives for that seed alone."""
+    from paper_1605_02620_b200 import timeseries
+    cfg = dict(L=256, N=1, R=3, tile=64, subsweeps=1)
+    seeds, times = (1, 2, 3, 4), [1, 2, 5, 9]
+    buf = io.StringIO()
+    ts, W2 = timeseries.run_seeds(rsos, cfg, seeds, times, out=buf)
+    rows = [json.loads(l) for l in buf.getvalue().splitlines()][1:]
+    assert len(rows) == len(seeds) * len(times) * cfg["R"] and W2.shape == (4, 4, 3)
+    got = {(row["seed"], row["t"], row["r"]): (row["S1"], row["S2"], row["accepted"]) for row in rows}
+    for i, sd in enumerate(seeds):
+        o = oracle_mod.Oracle(cfg["L"], cfg["N"], cfg["R"], sd, tile=cfg["tile"], subsweeps=cfg["subsweeps"])
+        t = 0
+        for j, tm in enumerate(times):
+            o.advance(tm - t)
+            t = tm
+            S1, S2, acc = o.sums()
+            assert (W2[i, j] == o.width()[0]).all()
+            for r in range(cfg["R"]):
+                assert got[(sd, tm, r)] == (int(S1[r]), int(S2[r]), int(acc[r])), (sd, tm, r)
+        o.close()
+
+
 def test_shape_measures_equal_oracle_on_a_reduced_steady_state(rsos, oracle_mod):
     """L = 32 (serial RS), 48 realizations, steady state from t = 400 (20 L^1.6 = 5120 is the config's rule; the width
     of an L = 32 surface saturates by t ~ 300), 12 samples: W^2 and the per-surface Phi^n from the GPU equal the
